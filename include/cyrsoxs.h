@@ -1,0 +1,176 @@
+/*
+ * cyrsoxs.h -- C ABI of libcyrsoxs, the B200 (sm_100a) forward-simulation hot path of
+ * CyRSoXS (arXiv 2209.13121).  Citations: P:n = PAPER.md line n; "DESIGN 3-Ax" = the
+ * reading of the paper fixed in DESIGN.md section 3.
+ *
+ * What one cyrsoxs_run computes (Algorithm 1), for every energy E_i and every
+ * in-plane E-field angle zeta of E_Angle[start, increment, end]:
+ *   1. induced polarization per voxel, Eq. 2-5:
+ *        p = (1/4pi) sum_m phi_m [ S_m ((n_perp^2-1) e + (n_par^2-n_perp^2)(d_m.e) d_m)
+ *                                  + (1-S_m)(n_iso^2-1) e ],
+ *        e = (cos zeta, sin zeta, 0), d = (cos psi sin theta, sin psi sin theta, cos theta),
+ *        n = 1 - delta + i beta, n_iso = (n_par + 2 n_perp)/3;
+ *   2. p~ = FFT(p), Eq. 6, forward, unnormalised, origin at voxel 0;
+ *   3. X = |k^2 (I - r r^T) p~|^2 on the Ewald sphere, Eq. 7-8:
+ *        q_z = sqrt(k^2 - q_x^2 - q_y^2) - k, k = 2 pi E / 1239.84197 nm^-1, real q_z only,
+ *        X taken at the nearest k_z bin or interpolated linearly between the two neighbours;
+ *   4. the image of each angle rotated back by -zeta about q = 0 (bilinear) and averaged over
+ *      the angles with per-pixel valid counts.
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback.
+ *
+ * Layouts.  Voxel (x, y, z) of a morphology array is element x + Nx (y + Ny z) (x fastest).
+ * Output pixel (iy, ix) of energy i is out[(i Ny + iy) Nx + ix] and corresponds to
+ * (q_x, q_y) = ((ix - Nx/2) dq_x, (iy - Ny/2) dq_y), dq = 2 pi / (N voxel_nm); q = 0 sits at
+ * (Ny/2, Nx/2).  Pixels that are valid at no angle are written as 0.0f.
+ *
+ * Threading: a context is not thread-safe; use one context per host thread / per GPU.
+ * Every function returns a status and never throws, aborts or prints.
+ */
+#ifndef CYRSOXS_H
+#define CYRSOXS_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cyrsoxs_ctx cyrsoxs_ctx; /* opaque; created and destroyed by the library */
+
+typedef enum {
+    CYRSOXS_OK = 0,
+    CYRSOXS_ERR_INVALID_ARG = 1,     /* bad size, NULL where not allowed, bad enum, bad angle spec */
+    CYRSOXS_ERR_NOT_READY = 2,       /* run before all of: morphology, optical constants, angles    */
+    CYRSOXS_ERR_CUDA = 3,            /* a CUDA call failed; cyrsoxs_last_error has the CUDA string  */
+    CYRSOXS_ERR_OOM = 4,             /* device (or pinned host) memory exhausted                    */
+    CYRSOXS_ERR_NOT_IMPLEMENTED = 5
+} cyrsoxs_status;
+
+typedef enum {
+    CYRSOXS_EWALD_NEAREST = 0,       /* X at k_z = floor(q_z/dq_z + 0.5) (north_star; not in the paper) */
+    CYRSOXS_EWALD_TRILINEAR = 1      /* X interpolated linearly between floor and floor+1      */
+} cyrsoxs_ewald;
+
+/* How the per-energy work is organised; all choices give the same images (tests check it).
+ *   PER_ENERGY      the paper's order with p linear in e (north_star): per energy the five
+ *                   distinct entries of the susceptibility tensor chi (xx, xy, xz, yy, yz; p for
+ *                   e = x is its first column, for e = y its second) are formed per voxel,
+ *                   transformed, and projected.
+ *   SPECTRAL_BASIS  p is also linear in the optical constants: the energy-independent real
+ *                   fields phi, phi S, phi S d_i d_j are transformed once per run and every
+ *                   energy only combines their spectra on its Ewald shell (DESIGN 7.2).
+ *   AUTO            picks whichever moves fewer bytes for the configured run. */
+typedef enum {
+    CYRSOXS_ALG_AUTO = 0,
+    CYRSOXS_ALG_PER_ENERGY = 1,
+    CYRSOXS_ALG_SPECTRAL_BASIS = 2
+} cyrsoxs_algorithm;
+
+/* Stage ids for cyrsoxs_stage_times / cyrsoxs_debug_fetch. */
+typedef enum {
+    CYRSOXS_STAGE_XPASS = 0,   /* polarization (or basis fields) fused with the FFT along x  */
+    CYRSOXS_STAGE_ZPASS = 1,   /* FFT along z, pruned to the k_z planes the Ewald shells touch */
+    CYRSOXS_STAGE_YPASS = 2,   /* FFT along y, pruned to |k_y| <= k/dq_y                       */
+    CYRSOXS_STAGE_EWALD = 3,   /* Ewald gather + (I - r r^T) + |.|^2 -> (I_xx, I_yy, I_xy, valid) */
+    CYRSOXS_STAGE_ROTATE = 4,  /* rotate back by -zeta, accumulate over angles, divide by counts */
+    CYRSOXS_N_STAGES = 5
+} cyrsoxs_stage;
+
+typedef struct {
+    int algorithm;                 /* cyrsoxs_algorithm actually used by the last run           */
+    int n_energy, n_angles;
+    int energy_batch;              /* energies processed per kernel launch group                */
+    long long kernel_launches;     /* kernels launched by the last run                          */
+    long long stage_launches[CYRSOXS_N_STAGES];
+    double stage_bytes[CYRSOXS_N_STAGES];   /* algorithmic HBM bytes per stage, whole run (DESIGN 8) */
+    float stage_ms[CYRSOXS_N_STAGES];       /* device time per stage, whole run; 0 unless profiling  */
+    double workspace_bytes;        /* device scratch owned by the context                       */
+} cyrsoxs_stats;
+
+/* Creates a context for an Nx x Ny x Nz voxel model with n_mat materials and cubic voxels of
+ * edge voxel_nm ("voxels are considered perfect cubes").  Sizes must be powers of two,
+ * 1 <= Nz, 2 <= Nx, Ny <= 4096, Nz <= 4096, 1 <= n_mat <= 32, voxel_nm > 0 (else
+ * INVALID_ARG).  Uses the current CUDA device.  *out is NULL on failure. */
+cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm, cyrsoxs_ctx **out);
+
+/* Morphology (memory model P:199-203): for each material m four DEVICE arrays of
+ * Nx*Ny*Nz float32: volume fraction phi (the paper's v_frac), alignment S, and the director's
+ * polar angle theta (from +z) and azimuth psi (from +x), radians.  d_phi etc. are HOST arrays
+ * of n_mat device pointers.  d_S[m], d_theta[m], d_psi[m] may all be NULL together for an
+ * isotropic material (S == 0); d_S, d_theta, d_psi themselves may be NULL if every material
+ * is isotropic.  Pointers are BORROWED: the caller keeps the arrays alive and unmodified until
+ * every run that uses them has completed.  Arrays must be 16-byte aligned.  The library does
+ * not check sum_m phi_m = 1 (neither does the paper's code) nor clamp S. */
+cyrsoxs_status cyrsoxs_set_morphology(cyrsoxs_ctx *ctx, const float *const *d_phi,
+                                      const float *const *d_S, const float *const *d_theta,
+                                      const float *const *d_psi);
+
+/* Same, from HOST arrays (pinned or pageable): copied into device buffers owned by the context
+ * with cudaMemcpyAsync on `cuda_stream` (the paper's one-off M_GPU <- M_CPU, Alg. 1 line 1,
+ * P:220).  The host arrays must stay valid until that stream reaches the end of the copy. */
+cyrsoxs_status cyrsoxs_set_morphology_host(cyrsoxs_ctx *ctx, const float *const *h_phi,
+                                           const float *const *h_S, const float *const *h_theta,
+                                           const float *const *h_psi, void *cuda_stream);
+
+/* Energy list and the material library: HOST arrays, copied.  energies_eV has
+ * n_energy entries (> 0); the four tables are [n_energy][n_mat] float32 with
+ * n_par = 1 - delta_par + i beta_par, n_perp likewise.  The complex coefficients
+ * n_perp^2 - 1, n_par^2 - n_perp^2, n_iso^2 - 1 are formed here in double as (n-1)(n+1) and
+ * rounded once to float32. */
+cyrsoxs_status cyrsoxs_set_optical_constants(cyrsoxs_ctx *ctx, int n_energy, const double *energies_eV,
+                                             const float *delta_par, const float *beta_par,
+                                             const float *delta_perp, const float *beta_perp);
+
+/* E_Angle[start, increment, end] in degrees: zeta_n = start + n step for
+ * n = 0 .. floor((end - start)/step + 1e-9); start == end gives one angle.  INVALID_ARG for
+ * step == 0 with start != end, for (end - start)/step < 0, or for more than 4096 angles. */
+cyrsoxs_status cyrsoxs_set_angles(cyrsoxs_ctx *ctx, double start_deg, double step_deg, double end_deg);
+
+/* Ewald interpolation along q_z; default CYRSOXS_EWALD_TRILINEAR (the paper's). */
+cyrsoxs_status cyrsoxs_set_ewald(cyrsoxs_ctx *ctx, cyrsoxs_ewald mode);
+
+/* Work organisation; default CYRSOXS_ALG_AUTO. */
+cyrsoxs_status cyrsoxs_set_algorithm(cyrsoxs_ctx *ctx, cyrsoxs_algorithm alg);
+
+/* Optional second output of cyrsoxs_run: per-pixel number of angles that contributed,
+ * n_energy*Ny*Nx unsigned ints in DEVICE memory, same layout as out.  NULL (default) disables. */
+cyrsoxs_status cyrsoxs_set_counts_output(cyrsoxs_ctx *ctx, unsigned int *d_counts);
+
+/* When enabled, each run brackets every stage with CUDA events and cyrsoxs_get_stats reports
+ * stage_ms (this serialises the internal streams a little; keep it off for throughput runs). */
+cyrsoxs_status cyrsoxs_set_profiling(cyrsoxs_ctx *ctx, int enabled);
+
+/* Runs the whole path for all energies and angles.  All work is enqueued on `cuda_stream`
+ * (a cudaStream_t; NULL = the legacy default stream) and on internal streams fenced to it by
+ * events; the call returns without synchronising, and `out` is complete when `cuda_stream`
+ * reaches the point after the call.  `out` is n_energy*Ny*Nx float32 in DEVICE memory, or in
+ * PINNED HOST memory (then each energy batch's images are copied back asynchronously while
+ * the next batch computes, "the averaged result is transferred from GPU to CPU").
+ * Scratch is allocated on first use and kept by the context (ERR_OOM if it does not fit). */
+cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *ctx, void *cuda_stream, float *out);
+
+/* Number of angles currently configured (0 before cyrsoxs_set_angles). */
+int cyrsoxs_num_angles(const cyrsoxs_ctx *ctx);
+
+/* Counters of the last run (see cyrsoxs_stats).  Synchronises `cuda_stream` of that run if
+ * profiling is enabled. */
+cyrsoxs_status cyrsoxs_get_stats(cyrsoxs_ctx *ctx, cyrsoxs_stats *stats);
+
+/* Test hook, not part of the contract: copies the per-energy Ewald images of the LAST energy
+ * batch of the last run, as float4 (I_xx, I_yy, I_xy, valid) per pixel, for batch-local energy
+ * index `e_in_batch`, into d_dst (Ny*Nx*4 floats, device).  Enqueued on the run's stream. */
+cyrsoxs_status cyrsoxs_debug_fetch_images(cyrsoxs_ctx *ctx, int e_in_batch, float *d_dst);
+
+/* Human-readable description of the last error of this context ("" if none).  The string is
+ * owned by the context and valid until the next call on it.  Accepts NULL (returns a static
+ * string describing a creation failure). */
+const char *cyrsoxs_last_error(const cyrsoxs_ctx *ctx);
+
+/* Frees the context and its scratch; borrowed morphology arrays are left alone.  NULL is ok. */
+void cyrsoxs_destroy(cyrsoxs_ctx *ctx);
+
+/* Library version string, e.g. "cyrsoxs-b200 0.1 (sm_100a)". */
+const char *cyrsoxs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CYRSOXS_H */

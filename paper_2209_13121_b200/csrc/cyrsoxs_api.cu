@@ -1,0 +1,687 @@
+// cyrsoxs_api.cu -- C ABI (include/cyrsoxs.h) and host driver of the CyRSoXS hot path.
+// The driver only validates, sizes buffers, computes a few per-energy scalars in double
+// (k and the complex coefficients, Eq. 1 / north_star) and launches the
+// kernels of kernels.cuh; every step of the path runs on the device.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+#include <algorithm>
+#include <complex>
+#include <string>
+#include <vector>
+
+#include "../../include/cyrsoxs.h"
+#include "kernels.cuh"
+
+using namespace cyr;
+
+namespace {
+
+constexpr double kPi = 3.141592653589793;
+constexpr double kHcEvNm = 1239.84197;
+constexpr int kMaxAngles = 4096;
+constexpr int kMaxLog2 = 11;
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+};
+
+} // namespace
+
+struct cyrsoxs_ctx {
+    int Nx = 0, Ny = 0, Nz = 0, n_mat = 0, device = 0;
+    float voxel = 0.f;
+    double dqx = 0, dqy = 0, dqz = 0;
+    // morphology
+    MorphPtrs mp{};
+    bool have_morph = false;
+    std::vector<void *> owned_morph;
+    // optics
+    int nE = 0;
+    std::vector<double> energies, k;
+    std::vector<float> coef;           // [nE][n_mat][6]: Cc, Ca, Cb (complex) / 4 pi
+    DevBuf d_coef, d_k;
+    bool have_optics = false;
+    // angles
+    int nA = 0;
+    std::vector<double2> cs;
+    DevBuf d_cs, d_csf;
+    bool have_angles = false;
+    // options
+    int ewald = CYRSOXS_EWALD_TRILINEAR;
+    int alg = CYRSOXS_ALG_AUTO;
+    int profiling = 0;
+    unsigned int *d_counts = nullptr;
+    // workspace
+    DevBuf A1, A2, A3, img, twx, twy, twz, stage_out[2];
+    void *pinned_probe = nullptr;
+    // last run
+    cyrsoxs_stats stats{};
+    cudaStream_t last_stream = nullptr;
+    int last_batch_e = 0;
+    std::vector<cudaEvent_t> prof_events;          // pairs (start, stop) tagged by stage
+    std::vector<int> prof_stage;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_batch[2] = {nullptr, nullptr}, ev_copy[2] = {nullptr, nullptr};
+    std::string err;
+};
+
+namespace {
+
+const char *kCreateFailed = "cyrsoxs_create failed (invalid argument, no CUDA device or out of memory)";
+
+cyrsoxs_status fail(cyrsoxs_ctx *c, cyrsoxs_status st, const char *fmt, ...)
+{
+    if (c) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        c->err = buf;
+    }
+    return st;
+}
+
+#define CUDA_TRY(c, expr)                                                                         \
+    do {                                                                                          \
+        cudaError_t _e = (expr);                                                                  \
+        if (_e != cudaSuccess) {                                                                  \
+            cudaGetLastError();                                                                   \
+            return fail((c), _e == cudaErrorMemoryAllocation ? CYRSOXS_ERR_OOM : CYRSOXS_ERR_CUDA, \
+                        "%s: %s", #expr, cudaGetErrorString(_e));                                 \
+        }                                                                                         \
+    } while (0)
+
+bool is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
+int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+
+cyrsoxs_status ensure(cyrsoxs_ctx *c, DevBuf &b, size_t bytes)
+{
+    if (bytes <= b.cap) return CYRSOXS_OK;
+    if (b.p) { cudaFree(b.p); b.p = nullptr; b.cap = 0; }
+    cudaError_t e = cudaMalloc(&b.p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        b.p = nullptr;
+        return fail(c, CYRSOXS_ERR_OOM, "cudaMalloc(%zu bytes): %s", bytes, cudaGetErrorString(e));
+    }
+    b.cap = bytes;
+    return CYRSOXS_OK;
+}
+
+void release(DevBuf &b)
+{
+    if (b.p) cudaFree(b.p);
+    b.p = nullptr; b.cap = 0;
+}
+
+// exp(-2 pi i t / N), t < N, evaluated in double and rounded once.
+cyrsoxs_status make_twiddles(cyrsoxs_ctx *c, DevBuf &b, int N)
+{
+    std::vector<float2> h((size_t)std::max(N, 1));
+    for (int t = 0; t < N; ++t) {
+        double ang = -2.0 * kPi * (double)t / (double)N;
+        h[t] = make_float2((float)cos(ang), (float)sin(ang));
+    }
+    // exact values on the axes
+    if (N >= 4) { h[N / 4] = make_float2(0.f, -1.f); h[N / 2] = make_float2(-1.f, 0.f); h[3 * N / 4] = make_float2(0.f, 1.f); }
+    else if (N == 2) h[1] = make_float2(-1.f, 0.f);
+    cyrsoxs_status st = ensure(c, b, sizeof(float2) * h.size());
+    if (st != CYRSOXS_OK) return st;
+    CUDA_TRY(c, cudaMemcpy(b.p, h.data(), sizeof(float2) * h.size(), cudaMemcpyHostToDevice));
+    return CYRSOXS_OK;
+}
+
+// Window of bins [-K, K] (symmetric) or [-K, 0] (one-sided) on an axis of length N.
+Window make_window(int N, int K, bool symmetric)
+{
+    Window w;
+    w.N = N;
+    int width = symmetric ? 2 * K + 1 : K + 1;
+    if (width >= N) { w.lo = -(N / 2); w.W = N; }
+    else { w.lo = -K; w.W = width; }
+    return w;
+}
+
+int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+struct Plan {
+    Window wx, wy, wz;
+    int pitch;
+    int eb;                    // energies per batch
+    size_t a1, a2, a3, img;    // float2 / float2 / float2 / float4 element counts per batch
+};
+
+// Windows from the largest wavenumber in [e0, e1): valid pixels have |q_x|, |q_y| <= k and
+// k_z nodes in [-(k/dq_z) - 1, 0] (Eq. 8).  One extra bin of slack on every side.
+void windows_for(const cyrsoxs_ctx *c, double kmax, Window &wx, Window &wy, Window &wz, int &pitch)
+{
+    int Kx = (int)floor(kmax / c->dqx) + 1, Ky = (int)floor(kmax / c->dqy) + 1;
+    wx = make_window(c->Nx, Kx, true);
+    wy = make_window(c->Ny, Ky, true);
+    if (c->Nz == 1) { wz.N = 1; wz.lo = 0; wz.W = 1; }
+    else { int Kz = (int)floor(kmax / c->dqz) + 2; wz = make_window(c->Nz, Kz, false); }
+    pitch = round_up(wx.W, 32);
+}
+
+template <int LOGN> cyrsoxs_status launch_xpass_t(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, float2 *out,
+                                                  const Window &wx, int pitch)
+{
+    using Cfg = XCfg<LOGN>;
+    static bool attr_done[64] = {false};
+    if (!attr_done[c->device & 63]) {
+        CUDA_TRY(c, cudaFuncSetAttribute(k_xpass_chi<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        attr_done[c->device & 63] = true;
+    }
+    const int rows = c->Ny * c->Nz;
+    dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS, eb);
+    k_xpass_chi<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(c->mp, (const float *)c->d_coef.p, e0, out, rows, wx, pitch,
+                                                             (const float2 *)c->twx.p);
+    CUDA_TRY(c, cudaGetLastError());
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status launch_xpass(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, float2 *out, const Window &wx, int pitch)
+{
+    switch (ilog2(c->Nx)) {
+#define CASE(L) case L: return launch_xpass_t<L>(c, st, e0, eb, out, wx, pitch);
+        CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11)
+#undef CASE
+    }
+    return fail(c, CYRSOXS_ERR_INVALID_ARG, "unsupported Nx");
+}
+
+template <int LOGN> cyrsoxs_status launch_colpass_t(cyrsoxs_ctx *c, cudaStream_t st, ColParams p, int n_lo, int n_hi, int pitch)
+{
+    using Cfg = ColCfg<LOGN>;
+    static bool attr_done[64] = {false};
+    if (!attr_done[c->device & 63]) {
+        CUDA_TRY(c, cudaFuncSetAttribute(k_colpass<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        attr_done[c->device & 63] = true;
+    }
+    p.n_tiles = pitch / Cfg::TX;
+    dim3 grid((unsigned)(p.n_tiles * n_lo), (unsigned)n_hi);
+    k_colpass<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    CUDA_TRY(c, cudaGetLastError());
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status launch_colpass(cyrsoxs_ctx *c, cudaStream_t st, int N, const ColParams &p, int n_lo, int n_hi, int pitch)
+{
+    switch (ilog2(N)) {
+#define CASE(L) case L: return launch_colpass_t<L>(c, st, p, n_lo, n_hi, pitch);
+        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11)
+#undef CASE
+    }
+    return fail(c, CYRSOXS_ERR_INVALID_ARG, "unsupported transform length %d", N);
+}
+
+struct StageTimer {
+    cyrsoxs_ctx *c;
+    cudaStream_t st;
+    int stage;
+    cudaEvent_t a = nullptr, b = nullptr;
+    StageTimer(cyrsoxs_ctx *c_, cudaStream_t s, int stage_) : c(c_), st(s), stage(stage_)
+    {
+        c->stats.stage_launches[stage]++;
+        c->stats.kernel_launches++;
+        if (c->profiling) {
+            cudaEventCreate(&a); cudaEventCreate(&b);
+            cudaEventRecord(a, st);
+        }
+    }
+    ~StageTimer()
+    {
+        if (c->profiling) {
+            cudaEventRecord(b, st);
+            c->prof_events.push_back(a); c->prof_events.push_back(b);
+            c->prof_stage.push_back(stage);
+        }
+    }
+};
+
+void clear_prof(cyrsoxs_ctx *c)
+{
+    for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
+    c->prof_events.clear();
+    c->prof_stage.clear();
+}
+
+// One energy batch of the PER_ENERGY algorithm: fields -> x -> z -> y -> Ewald -> rotate.
+cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, float *d_out, unsigned int *d_cnt)
+{
+    double kmax = 0;
+    for (int e = e0; e < e0 + eb; ++e) kmax = std::max(kmax, c->k[e]);
+    Window wx, wy, wz;
+    int pitch;
+    windows_for(c, kmax, wx, wy, wz, pitch);
+    const int F = NCHI * eb;
+    const size_t rows = (size_t)c->Ny * c->Nz;
+    float2 *A1 = (float2 *)c->A1.p, *A2 = (float2 *)c->A2.p, *A3 = (float2 *)c->A3.p;
+    cyrsoxs_status s;
+    double n_iso = 0, n_al = 0;
+    for (int m = 0; m < c->n_mat; ++m) (c->mp.S[m] ? n_al : n_iso) += 1;
+    const double nvox = (double)c->Nx * c->Ny * c->Nz;
+    {
+        StageTimer t(c, st, CYRSOXS_STAGE_XPASS);
+        if ((s = launch_xpass(c, st, e0, eb, A1, wx, pitch)) != CYRSOXS_OK) return s;
+        c->stats.stage_bytes[CYRSOXS_STAGE_XPASS] += eb * nvox * (16.0 * n_al + 4.0 * n_iso) + 8.0 * F * rows * pitch;
+    }
+    const float2 *ysrc = A1;
+    if (c->Nz > 1) {
+        StageTimer t(c, st, CYRSOXS_STAGE_ZPASS);
+        ColParams p{};
+        p.in = A1; p.out = A2;
+        p.in_row = (long long)c->Ny * pitch; p.out_row = (long long)c->Ny * pitch;
+        p.in_lo = pitch; p.out_lo = pitch;
+        p.in_hi = (long long)c->Nz * c->Ny * pitch; p.out_hi = (long long)wz.W * c->Ny * pitch;
+        p.win = wz; p.tw = (const float2 *)c->twz.p;
+        if ((s = launch_colpass(c, st, c->Nz, p, c->Ny, F, pitch)) != CYRSOXS_OK) return s;
+        c->stats.stage_bytes[CYRSOXS_STAGE_ZPASS] += 8.0 * F * c->Ny * pitch * ((double)c->Nz + wz.W);
+        ysrc = A2;
+    }
+    {
+        StageTimer t(c, st, CYRSOXS_STAGE_YPASS);
+        ColParams p{};
+        p.in = ysrc; p.out = A3;
+        p.in_row = pitch; p.out_row = pitch;
+        p.in_lo = (long long)c->Ny * pitch; p.out_lo = (long long)wy.W * pitch;
+        p.in_hi = (long long)wz.W * c->Ny * pitch; p.out_hi = (long long)wz.W * wy.W * pitch;
+        p.win = wy; p.tw = (const float2 *)c->twy.p;
+        if ((s = launch_colpass(c, st, c->Ny, p, wz.W, F, pitch)) != CYRSOXS_OK) return s;
+        c->stats.stage_bytes[CYRSOXS_STAGE_YPASS] += 8.0 * F * wz.W * pitch * ((double)c->Ny + wy.W);
+    }
+    dim3 g2((c->Nx + 31) / 32, (c->Ny + 7) / 8, eb);
+    {
+        StageTimer t(c, st, CYRSOXS_STAGE_EWALD);
+        EwaldParams p{};
+        p.Nx = c->Nx; p.Ny = c->Ny; p.Nz = c->Nz; p.mode = c->ewald;
+        p.dqx = c->dqx; p.dqy = c->dqy; p.dqz = c->dqz;
+        p.k = (const double *)c->d_k.p; p.e0 = e0;
+        p.wx = wx; p.wy = wy; p.wz = wz; p.pitch = pitch;
+        p.spec = A3; p.img = (float4 *)c->img.p;
+        k_ewald_chi<<<g2, 256, 0, st>>>(p);
+        CUDA_TRY(c, cudaGetLastError());
+        const double nodes = (c->Nz > 1 && c->ewald == CYRSOXS_EWALD_TRILINEAR) ? 2.0 : 1.0;
+        c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * 0.785 * nodes * NCHI * 8.0 + 16.0 * c->Nx * c->Ny);
+    }
+    {
+        StageTimer t(c, st, CYRSOXS_STAGE_ROTATE);
+        RotateParams p{};
+        p.Nx = c->Nx; p.Ny = c->Ny; p.n_angles = c->nA;
+        p.cs = (const double2 *)c->d_cs.p; p.csf = (const float4 *)c->d_csf.p;
+        p.img = (const float4 *)c->img.p; p.out = d_out; p.counts = d_cnt;
+        k_rotate_avg<<<g2, 256, 0, st>>>(p);
+        CUDA_TRY(c, cudaGetLastError());
+        c->stats.stage_bytes[CYRSOXS_STAGE_ROTATE] += eb * (20.0 * c->Nx * c->Ny);
+    }
+    return CYRSOXS_OK;
+}
+
+} // namespace
+
+// =========================================================================================
+
+extern "C" {
+
+const char *cyrsoxs_version(void) { return "cyrsoxs-b200 0.1 (sm_100a)"; }
+
+const char *cyrsoxs_last_error(const cyrsoxs_ctx *ctx) { return ctx ? ctx->err.c_str() : kCreateFailed; }
+
+cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm, cyrsoxs_ctx **out)
+{
+    if (!out) return CYRSOXS_ERR_INVALID_ARG;
+    *out = nullptr;
+    const int maxn = 1 << kMaxLog2;
+    if (!is_pow2(Nx) || !is_pow2(Ny) || !is_pow2(Nz) || Nx < 4 || Ny < 2 || Nz < 1 || Nx > maxn || Ny > maxn || Nz > maxn)
+        return CYRSOXS_ERR_INVALID_ARG;
+    if (n_mat < 1 || n_mat > MAX_MAT || !(voxel_nm > 0.f) || !isfinite(voxel_nm)) return CYRSOXS_ERR_INVALID_ARG;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CYRSOXS_ERR_CUDA; }
+    cyrsoxs_ctx *c = new (std::nothrow) cyrsoxs_ctx();
+    if (!c) return CYRSOXS_ERR_OOM;
+    c->Nx = Nx; c->Ny = Ny; c->Nz = Nz; c->n_mat = n_mat; c->voxel = voxel_nm; c->device = dev;
+    c->dqx = (2.0 * kPi) / ((double)Nx * (double)voxel_nm);
+    c->dqy = (2.0 * kPi) / ((double)Ny * (double)voxel_nm);
+    c->dqz = (2.0 * kPi) / ((double)Nz * (double)voxel_nm);
+    c->mp.n_mat = n_mat;
+    cyrsoxs_status st;
+    if ((st = make_twiddles(c, c->twx, Nx)) != CYRSOXS_OK || (st = make_twiddles(c, c->twy, Ny)) != CYRSOXS_OK
+        || (st = make_twiddles(c, c->twz, Nz)) != CYRSOXS_OK) {
+        cyrsoxs_destroy(c);
+        return st;
+    }
+    *out = c;
+    return CYRSOXS_OK;
+}
+
+void cyrsoxs_destroy(cyrsoxs_ctx *c)
+{
+    if (!c) return;
+    clear_prof(c);
+    for (void *p : c->owned_morph) cudaFree(p);
+    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_cs, &c->d_csf, &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
+                      &c->stage_out[0], &c->stage_out[1]})
+        release(*b);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    for (int i = 0; i < 2; ++i) {
+        if (c->ev_batch[i]) cudaEventDestroy(c->ev_batch[i]);
+        if (c->ev_copy[i]) cudaEventDestroy(c->ev_copy[i]);
+    }
+    delete c;
+}
+
+static cyrsoxs_status check_morph_tables(cyrsoxs_ctx *c, const float *const *phi, const float *const *S,
+                                         const float *const *theta, const float *const *psi)
+{
+    if (!phi) return fail(c, CYRSOXS_ERR_INVALID_ARG, "phi table is NULL");
+    for (int m = 0; m < c->n_mat; ++m) {
+        if (!phi[m]) return fail(c, CYRSOXS_ERR_INVALID_ARG, "phi[%d] is NULL", m);
+        const float *s = S ? S[m] : nullptr, *t = theta ? theta[m] : nullptr, *p = psi ? psi[m] : nullptr;
+        if ((s || t || p) && !(s && t && p))
+            return fail(c, CYRSOXS_ERR_INVALID_ARG, "material %d: S, theta, psi must be all set or all NULL", m);
+    }
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_morphology(cyrsoxs_ctx *c, const float *const *d_phi, const float *const *d_S,
+                                      const float *const *d_theta, const float *const *d_psi)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    cyrsoxs_status st = check_morph_tables(c, d_phi, d_S, d_theta, d_psi);
+    if (st != CYRSOXS_OK) return st;
+    for (int m = 0; m < c->n_mat; ++m) {
+        const float *ptrs[4] = {d_phi[m], d_S ? d_S[m] : nullptr, d_theta ? d_theta[m] : nullptr, d_psi ? d_psi[m] : nullptr};
+        for (const float *p : ptrs)
+            if (p && ((uintptr_t)p & 15)) return fail(c, CYRSOXS_ERR_INVALID_ARG, "material %d: array not 16-byte aligned", m);
+    }
+    for (int m = 0; m < c->n_mat; ++m) {
+        c->mp.phi[m] = d_phi[m];
+        c->mp.S[m] = d_S ? d_S[m] : nullptr;
+        c->mp.theta[m] = d_theta ? d_theta[m] : nullptr;
+        c->mp.psi[m] = d_psi ? d_psi[m] : nullptr;
+    }
+    c->have_morph = true;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_morphology_host(cyrsoxs_ctx *c, const float *const *h_phi, const float *const *h_S,
+                                           const float *const *h_theta, const float *const *h_psi, void *cuda_stream)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    cyrsoxs_status st = check_morph_tables(c, h_phi, h_S, h_theta, h_psi);
+    if (st != CYRSOXS_OK) return st;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t bytes = sizeof(float) * (size_t)c->Nx * c->Ny * c->Nz;
+    // count arrays, (re)allocate owned buffers
+    std::vector<const float *> src;
+    for (int m = 0; m < c->n_mat; ++m) {
+        src.push_back(h_phi[m]);
+        src.push_back(h_S ? h_S[m] : nullptr);
+        src.push_back(h_theta ? h_theta[m] : nullptr);
+        src.push_back(h_psi ? h_psi[m] : nullptr);
+    }
+    size_t need = 0;
+    for (const float *p : src) need += p ? 1 : 0;
+    if (c->owned_morph.size() != need) {
+        for (void *p : c->owned_morph) cudaFree(p);
+        c->owned_morph.clear();
+        for (size_t i = 0; i < need; ++i) {
+            void *d = nullptr;
+            cudaError_t e = cudaMalloc(&d, bytes);
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                for (void *p : c->owned_morph) cudaFree(p);
+                c->owned_morph.clear();
+                c->have_morph = false;
+                return fail(c, CYRSOXS_ERR_OOM, "cudaMalloc(morphology, %zu bytes): %s", bytes, cudaGetErrorString(e));
+            }
+            c->owned_morph.push_back(d);
+        }
+    }
+    size_t slot = 0;
+    const float *dptr[4 * MAX_MAT];
+    for (size_t i = 0; i < src.size(); ++i) {
+        dptr[i] = nullptr;
+        if (!src[i]) continue;
+        void *d = c->owned_morph[slot++];
+        CUDA_TRY(c, cudaMemcpyAsync(d, src[i], bytes, cudaMemcpyHostToDevice, s));
+        dptr[i] = (const float *)d;
+    }
+    for (int m = 0; m < c->n_mat; ++m) {
+        c->mp.phi[m] = dptr[4 * m]; c->mp.S[m] = dptr[4 * m + 1];
+        c->mp.theta[m] = dptr[4 * m + 2]; c->mp.psi[m] = dptr[4 * m + 3];
+    }
+    c->have_morph = true;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_optical_constants(cyrsoxs_ctx *c, int n_energy, const double *energies_eV,
+                                             const float *delta_par, const float *beta_par,
+                                             const float *delta_perp, const float *beta_perp)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (n_energy < 1 || !energies_eV || !delta_par || !beta_par || !delta_perp || !beta_perp)
+        return fail(c, CYRSOXS_ERR_INVALID_ARG, "optical constants: NULL table or n_energy < 1");
+    for (int e = 0; e < n_energy; ++e)
+        if (!(energies_eV[e] > 0.0) || !isfinite(energies_eV[e]))
+            return fail(c, CYRSOXS_ERR_INVALID_ARG, "energy %d is not positive", e);
+    const int M = c->n_mat;
+    c->nE = n_energy;
+    c->energies.assign(energies_eV, energies_eV + n_energy);
+    c->k.resize(n_energy);
+    c->coef.resize((size_t)n_energy * M * 6);
+    typedef std::complex<double> cd;
+    const double inv4pi = 1.0 / (4.0 * kPi);
+    for (int e = 0; e < n_energy; ++e) {
+        const double lambda = kHcEvNm / energies_eV[e];
+        c->k[e] = (2.0 * kPi) / lambda;
+        for (int m = 0; m < M; ++m) {
+            const size_t i = (size_t)e * M + m;
+            // n - 1 = -delta + i beta; n^2 - 1 = (n - 1)(n + 1): nothing of size 1 cancels
+            const cd npar(-(double)delta_par[i], (double)beta_par[i]), nperp(-(double)delta_perp[i], (double)beta_perp[i]);
+            const cd niso = (npar + 2.0 * nperp) / 3.0;
+            const cd a = nperp * (nperp + 2.0), b = (npar - nperp) * (npar + nperp + 2.0), cc = niso * (niso + 2.0);
+            // a - c = (n_perp - n_iso)(n_perp + n_iso), again without cancellation
+            const cd amc = (nperp - niso) * (nperp + niso + 2.0);
+            const cd Cc = cc * inv4pi, Ca = amc * inv4pi, Cb = b * inv4pi;
+            (void)a;
+            float *o = &c->coef[i * 6];
+            o[0] = (float)Cc.real(); o[1] = (float)Cc.imag();
+            o[2] = (float)Ca.real(); o[3] = (float)Ca.imag();
+            o[4] = (float)Cb.real(); o[5] = (float)Cb.imag();
+        }
+    }
+    cyrsoxs_status st;
+    if ((st = ensure(c, c->d_coef, sizeof(float) * c->coef.size())) != CYRSOXS_OK) return st;
+    if ((st = ensure(c, c->d_k, sizeof(double) * n_energy)) != CYRSOXS_OK) return st;
+    CUDA_TRY(c, cudaMemcpy(c->d_coef.p, c->coef.data(), sizeof(float) * c->coef.size(), cudaMemcpyHostToDevice));
+    CUDA_TRY(c, cudaMemcpy(c->d_k.p, c->k.data(), sizeof(double) * n_energy, cudaMemcpyHostToDevice));
+    c->have_optics = true;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_angles(cyrsoxs_ctx *c, double start_deg, double step_deg, double end_deg)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (!isfinite(start_deg) || !isfinite(step_deg) || !isfinite(end_deg))
+        return fail(c, CYRSOXS_ERR_INVALID_ARG, "angles must be finite");
+    int n;
+    if (start_deg == end_deg) n = 1;
+    else {
+        if (step_deg == 0.0) return fail(c, CYRSOXS_ERR_INVALID_ARG, "angle step is 0 with start != end");
+        double q = floor((end_deg - start_deg) / step_deg + 1e-9);
+        if (q < 0.0) return fail(c, CYRSOXS_ERR_INVALID_ARG, "(end - start)/step is negative");
+        if (q + 1.0 > (double)kMaxAngles) return fail(c, CYRSOXS_ERR_INVALID_ARG, "more than %d angles", kMaxAngles);
+        n = (int)q + 1;
+    }
+    c->nA = n;
+    c->cs.resize(n);
+    std::vector<float4> csf(n);
+    for (int i = 0; i < n; ++i) {
+        const double zeta = start_deg + (double)i * step_deg;
+        const double zr = zeta * (kPi / 180.0);
+        double C = cos(zr), S = sin(zr);
+        if (fabs(C) < 1e-15) C = 0.0;
+        if (fabs(S) < 1e-15) S = 0.0;
+        c->cs[i] = make_double2(C, S);
+        csf[i] = make_float4((float)(C * C), (float)(S * S), (float)(2.0 * C * S), 0.f);
+    }
+    cyrsoxs_status st;
+    if ((st = ensure(c, c->d_cs, sizeof(double2) * n)) != CYRSOXS_OK) return st;
+    if ((st = ensure(c, c->d_csf, sizeof(float4) * n)) != CYRSOXS_OK) return st;
+    CUDA_TRY(c, cudaMemcpy(c->d_cs.p, c->cs.data(), sizeof(double2) * n, cudaMemcpyHostToDevice));
+    CUDA_TRY(c, cudaMemcpy(c->d_csf.p, csf.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
+    c->have_angles = true;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_ewald(cyrsoxs_ctx *c, cyrsoxs_ewald mode)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (mode != CYRSOXS_EWALD_NEAREST && mode != CYRSOXS_EWALD_TRILINEAR) return fail(c, CYRSOXS_ERR_INVALID_ARG, "unknown Ewald mode");
+    c->ewald = mode;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_algorithm(cyrsoxs_ctx *c, cyrsoxs_algorithm alg)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (alg != CYRSOXS_ALG_AUTO && alg != CYRSOXS_ALG_PER_ENERGY && alg != CYRSOXS_ALG_SPECTRAL_BASIS)
+        return fail(c, CYRSOXS_ERR_INVALID_ARG, "unknown algorithm");
+    c->alg = alg;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_counts_output(cyrsoxs_ctx *c, unsigned int *d_counts)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    c->d_counts = d_counts;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_profiling(cyrsoxs_ctx *c, int enabled)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    c->profiling = enabled ? 1 : 0;
+    return CYRSOXS_OK;
+}
+
+int cyrsoxs_num_angles(const cyrsoxs_ctx *c) { return c && c->have_angles ? c->nA : 0; }
+
+cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (!out) return fail(c, CYRSOXS_ERR_INVALID_ARG, "out is NULL");
+    if (!c->have_morph || !c->have_optics || !c->have_angles)
+        return fail(c, CYRSOXS_ERR_NOT_READY, "run needs morphology, optical constants and angles (missing:%s%s%s)",
+                    c->have_morph ? "" : " morphology", c->have_optics ? "" : " optical-constants", c->have_angles ? "" : " angles");
+    if (c->alg == CYRSOXS_ALG_SPECTRAL_BASIS) return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "SPECTRAL_BASIS is not built yet");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+
+    // where does `out` live?
+    cudaPointerAttributes pa{};
+    cudaError_t pe = cudaPointerGetAttributes(&pa, out);
+    if (pe != cudaSuccess) { cudaGetLastError(); return fail(c, CYRSOXS_ERR_INVALID_ARG, "out: %s", cudaGetErrorString(pe)); }
+    const bool out_on_host = pa.type == cudaMemoryTypeHost;
+    if (pa.type != cudaMemoryTypeHost && pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
+        return fail(c, CYRSOXS_ERR_INVALID_ARG, "out must be device memory or pinned host memory");
+
+    // plan: windows for the largest k, energy batch from the free memory
+    double kmax = *std::max_element(c->k.begin(), c->k.end());
+    Window wx, wy, wz;
+    int pitch;
+    windows_for(c, kmax, wx, wy, wz, pitch);
+    const size_t npix = (size_t)c->Nx * c->Ny;
+    const size_t a1 = (size_t)NCHI * c->Nz * c->Ny * pitch, a2 = c->Nz > 1 ? (size_t)NCHI * wz.W * c->Ny * pitch : 0,
+                 a3 = (size_t)NCHI * wz.W * wy.W * pitch;
+    const size_t per_e = sizeof(float2) * (a1 + a2 + a3) + sizeof(float4) * npix + (out_on_host ? 2 * sizeof(float) * npix : 0);
+    size_t free_b = 0, total_b = 0;
+    CUDA_TRY(c, cudaMemGetInfo(&free_b, &total_b));
+    const size_t have = c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap;
+    const size_t budget = (size_t)((double)(free_b + have) * 0.85);
+    int eb = (int)std::min<size_t>((size_t)c->nE, std::max<size_t>(1, budget / per_e));
+    // keep batches small enough that several fit in flight and large enough to fill the GPU
+    const size_t target = (size_t)1 << 31;        // ~2 GiB of fields per batch is plenty of parallelism
+    eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / (sizeof(float2) * a1))));
+    eb = std::min(eb, 64);
+    cyrsoxs_status s;
+    if ((s = ensure(c, c->A1, sizeof(float2) * a1 * eb)) != CYRSOXS_OK) return s;
+    if (a2 && (s = ensure(c, c->A2, sizeof(float2) * a2 * eb)) != CYRSOXS_OK) return s;
+    if ((s = ensure(c, c->A3, sizeof(float2) * a3 * eb)) != CYRSOXS_OK) return s;
+    if ((s = ensure(c, c->img, sizeof(float4) * npix * eb)) != CYRSOXS_OK) return s;
+    if (out_on_host) {
+        for (int i = 0; i < 2; ++i)
+            if ((s = ensure(c, c->stage_out[i], sizeof(float) * npix * eb)) != CYRSOXS_OK) return s;
+        if (!c->copy_stream) CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            if (!c->ev_batch[i]) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_batch[i], cudaEventDisableTiming));
+            if (!c->ev_copy[i]) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_copy[i], cudaEventDisableTiming));
+        }
+    }
+
+    clear_prof(c);
+    memset(&c->stats, 0, sizeof c->stats);
+    c->stats.algorithm = CYRSOXS_ALG_PER_ENERGY;
+    c->stats.n_energy = c->nE; c->stats.n_angles = c->nA; c->stats.energy_batch = eb;
+    c->stats.workspace_bytes = (double)(c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap);
+    c->last_stream = st;
+
+    int nb = 0;
+    for (int e0 = 0; e0 < c->nE; e0 += eb, ++nb) {
+        const int n = std::min(eb, c->nE - e0);
+        unsigned int *cnt = c->d_counts ? c->d_counts + (size_t)e0 * npix : nullptr;
+        if (!out_on_host) {
+            if ((s = run_batch_per_energy(c, st, e0, n, out + (size_t)e0 * npix, cnt)) != CYRSOXS_OK) return s;
+        } else {
+            const int slot = nb & 1;
+            // the staging slot is free once the copy issued two batches ago has finished
+            if (nb >= 2) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_copy[slot], 0));
+            if ((s = run_batch_per_energy(c, st, e0, n, (float *)c->stage_out[slot].p, cnt)) != CYRSOXS_OK) return s;
+            CUDA_TRY(c, cudaEventRecord(c->ev_batch[slot], st));
+            CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_batch[slot], 0));
+            CUDA_TRY(c, cudaMemcpyAsync(out + (size_t)e0 * npix, c->stage_out[slot].p, sizeof(float) * npix * n,
+                                        cudaMemcpyDeviceToHost, c->copy_stream));
+            CUDA_TRY(c, cudaEventRecord(c->ev_copy[slot], c->copy_stream));
+        }
+        c->last_batch_e = n;
+    }
+    if (out_on_host) {
+        // `out` is complete when `st` reaches this point
+        for (int i = 0; i < std::min(nb, 2); ++i) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_copy[i], 0));
+    }
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_get_stats(cyrsoxs_ctx *c, cyrsoxs_stats *stats)
+{
+    if (!c || !stats) return CYRSOXS_ERR_INVALID_ARG;
+    if (c->profiling && !c->prof_events.empty()) {
+        CUDA_TRY(c, cudaStreamSynchronize(c->last_stream));
+        for (int i = 0; i < CYRSOXS_N_STAGES; ++i) c->stats.stage_ms[i] = 0.f;
+        for (size_t i = 0; i < c->prof_stage.size(); ++i) {
+            float ms = 0.f;
+            CUDA_TRY(c, cudaEventElapsedTime(&ms, c->prof_events[2 * i], c->prof_events[2 * i + 1]));
+            c->stats.stage_ms[c->prof_stage[i]] += ms;
+        }
+    }
+    *stats = c->stats;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_debug_fetch_images(cyrsoxs_ctx *c, int e_in_batch, float *d_dst)
+{
+    if (!c || !d_dst) return CYRSOXS_ERR_INVALID_ARG;
+    if (!c->img.p || e_in_batch < 0 || e_in_batch >= c->last_batch_e) return fail(c, CYRSOXS_ERR_INVALID_ARG, "no such image");
+    const size_t npix = (size_t)c->Nx * c->Ny;
+    CUDA_TRY(c, cudaMemcpyAsync(d_dst, (const float4 *)c->img.p + (size_t)e_in_batch * npix, sizeof(float4) * npix,
+                                cudaMemcpyDeviceToDevice, c->last_stream));
+    return CYRSOXS_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,382 @@
+// kernels.cuh -- the sm_100a kernels of the CyRSoXS hot path.
+//   k_xpass_chi   polarization (Eq. 2-5) fused with the FFT along x, pruned store
+//   k_colpass     strided FFT along z or y with a pruned, windowed store
+//   k_ewald_chi   Ewald gather (Eq. 8) + (I - r r^T) + |.|^2 (Eq. 7) -> (I_xx, I_yy, I_xy, valid)
+//   k_rotate_avg  rotate back by -zeta (bilinear), accumulate over angles, divide by counts
+// Geometry decisions use IEEE double with explicitly rounded operations (__dmul_rn ...), the
+// same sequence DESIGN.md 3-A11 writes out, so validity/cell decisions do not depend on FMA
+// contraction.  Values are float32.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "fft_core.cuh"
+
+namespace cyr {
+
+constexpr int MAX_MAT = 32;
+
+// Bins k in [lo, lo + W) (mod N) of a transformed axis are kept, bin k at slot (k - lo) mod N.
+struct Window {
+    int N, lo, W;
+};
+__host__ __device__ __forceinline__ int win_slot(const Window &w, int k) { return (k - w.lo) & (w.N - 1); }
+
+struct MorphPtrs {
+    const float *phi[MAX_MAT];
+    const float *S[MAX_MAT];
+    const float *theta[MAX_MAT];
+    const float *psi[MAX_MAT];
+    int n_mat;
+};
+
+// ------------------------------------------------------------------------------------------
+// x pass, PER_ENERGY algorithm.  One CTA = ROWS consecutive (y, z) rows x one energy.
+// Per voxel, with w = phi S and coefficients pre-divided by 4 pi (coef[e][m] = {Cc, Ca, Cb},
+// Cc = c/4pi, Ca = (a - c)/4pi, Cb = b/4pi, a = n_perp^2-1, b = n_par^2-n_perp^2, c = n_iso^2-1):
+//   chi_xx = sum_m Cc phi + Ca w + Cb w dx dx      chi_xy = sum_m Cb w dx dy
+//   chi_yy = sum_m Cc phi + Ca w + Cb w dy dy      chi_xz = sum_m Cb w dx dz
+//                                                   chi_yz = sum_m Cb w dy dz
+// which is Eq. 5's p for e = x (chi_xx, chi_xy, chi_xz) and e = y (chi_xy, chi_yy, chi_yz).
+// Output field f of energy e: out[((e*5 + f) * rows + row) * pitch + slot].
+constexpr int NCHI = 5;
+
+template <int LOGN> struct XCfg {
+    static constexpr int N = 1 << LOGN;
+    static constexpr int TPR = N / 4 > 0 ? N / 4 : 1;                    // threads per row (4 voxels each)
+    static constexpr int ROWS = TPR >= 256 ? 1 : 256 / TPR;              // rows per CTA
+    static constexpr int THREADS = TPR * ROWS;
+    static constexpr int NLINES = ROWS * NCHI;
+    static constexpr int LS = RowLayout<N>::LS;
+    static constexpr size_t SMEM = sizeof(float) * 2 * (size_t)NLINES * LS + sizeof(float2) * N
+                                   + sizeof(float) * 6 * MAX_MAT;
+};
+
+template <int LOGN>
+__global__ void __launch_bounds__(XCfg<LOGN>::THREADS)
+k_xpass_chi(const __grid_constant__ MorphPtrs mp, const float *__restrict__ coef, int e0,
+            float2 *__restrict__ out, int rows_total, Window wx, int pitch,
+            const float2 *__restrict__ tw_g)
+{
+    using Cfg = XCfg<LOGN>;
+    constexpr int N = Cfg::N;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float *re = reinterpret_cast<float *>(smem_raw);
+    float *im = re + Cfg::NLINES * Cfg::LS;
+    float2 *tw = reinterpret_cast<float2 *>(im + Cfg::NLINES * Cfg::LS);
+    float *cf = reinterpret_cast<float *>(tw + N);
+
+    const int tid = threadIdx.x;
+    const int e = blockIdx.y;
+    const int row0 = blockIdx.x * Cfg::ROWS;
+    const int nrows = min(Cfg::ROWS, rows_total - row0);
+    const int n_mat = mp.n_mat;
+
+    for (int i = tid; i < N; i += Cfg::THREADS) tw[i] = tw_g[i];
+    for (int i = tid; i < 6 * n_mat; i += Cfg::THREADS) cf[i] = coef[(size_t)(e0 + e) * 6 * n_mat + i];
+    __syncthreads();
+
+    const int rr = tid / Cfg::TPR, tx = tid % Cfg::TPR;
+    if (rr < nrows) {
+        float acc[4][2 * NCHI];
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+#pragma unroll
+            for (int q = 0; q < 2 * NCHI; ++q) acc[v][q] = 0.f;
+        const size_t base = (size_t)(row0 + rr) * N + 4 * tx;
+        constexpr int NV = N >= 4 ? 4 : N;
+        for (int m = 0; m < n_mat; ++m) {
+            const float ccr = cf[6 * m], cci = cf[6 * m + 1], car = cf[6 * m + 2], cai = cf[6 * m + 3],
+                        cbr = cf[6 * m + 4], cbi = cf[6 * m + 5];
+            float ph[4], s[4], th[4], ps[4];
+            const bool aligned = mp.S[m] != nullptr;
+            if (N >= 4) {
+                float4 t = __ldg(reinterpret_cast<const float4 *>(mp.phi[m] + base));
+                ph[0] = t.x; ph[1] = t.y; ph[2] = t.z; ph[3] = t.w;
+                if (aligned) {
+                    t = __ldg(reinterpret_cast<const float4 *>(mp.S[m] + base));
+                    s[0] = t.x; s[1] = t.y; s[2] = t.z; s[3] = t.w;
+                    t = __ldg(reinterpret_cast<const float4 *>(mp.theta[m] + base));
+                    th[0] = t.x; th[1] = t.y; th[2] = t.z; th[3] = t.w;
+                    t = __ldg(reinterpret_cast<const float4 *>(mp.psi[m] + base));
+                    ps[0] = t.x; ps[1] = t.y; ps[2] = t.z; ps[3] = t.w;
+                }
+            } else {
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    ph[v] = mp.phi[m][base + v];
+                    if (aligned) { s[v] = mp.S[m][base + v]; th[v] = mp.theta[m][base + v]; ps[v] = mp.psi[m][base + v]; }
+                }
+            }
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const float f = ph[v];
+                float dr = ccr * f, di = cci * f;           // diagonal (isotropic-like) part
+                if (aligned) {
+                    const float w = f * s[v];
+                    float st, ct, sp, cp;
+                    sincosf(th[v], &st, &ct);
+                    sincosf(ps[v], &sp, &cp);
+                    const float dx = cp * st, dy = sp * st, dz = ct;
+                    dr = fmaf(car, w, dr); di = fmaf(cai, w, di);
+                    const float br = cbr * w, bi = cbi * w;
+                    const float xx = dx * dx, yy = dy * dy, xy = dx * dy, xz = dx * dz, yz = dy * dz;
+                    acc[v][0] = fmaf(br, xx, acc[v][0]); acc[v][1] = fmaf(bi, xx, acc[v][1]);
+                    acc[v][2] = fmaf(br, xy, acc[v][2]); acc[v][3] = fmaf(bi, xy, acc[v][3]);
+                    acc[v][4] = fmaf(br, xz, acc[v][4]); acc[v][5] = fmaf(bi, xz, acc[v][5]);
+                    acc[v][6] = fmaf(br, yy, acc[v][6]); acc[v][7] = fmaf(bi, yy, acc[v][7]);
+                    acc[v][8] = fmaf(br, yz, acc[v][8]); acc[v][9] = fmaf(bi, yz, acc[v][9]);
+                }
+                acc[v][0] += dr; acc[v][1] += di;
+                acc[v][6] += dr; acc[v][7] += di;
+            }
+        }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            const int p = RowLayout<N>::input_pos(4 * tx + v);
+#pragma unroll
+            for (int f = 0; f < NCHI; ++f) {
+                const int o = (rr * NCHI + f) * Cfg::LS + p;
+                re[o] = acc[v][2 * f]; im[o] = acc[v][2 * f + 1];
+            }
+        }
+    }
+    __syncthreads();
+
+    RowAcc<N> racc{re, im};
+    fft_lines<LOGN, Cfg::NLINES, Cfg::THREADS>(racc, nrows * NCHI, tw, tid);
+
+    // pruned store: slot s <- bin (lo + s) mod N; pad columns [W, pitch) are zeroed
+    const int nl = nrows * NCHI;
+    const size_t fstride = (size_t)rows_total * pitch;
+    for (int idx = tid; idx < nl * pitch; idx += Cfg::THREADS) {
+        const int line = idx / pitch, sl = idx - line * pitch;
+        const int r = line / NCHI, f = line - r * NCHI;
+        float2 val = make_float2(0.f, 0.f);
+        if (sl < wx.W) {
+            const int b = (wx.lo + sl) & (N - 1);
+            const int p = line * Cfg::LS + RowLayout<N>::pos(b);
+            val = make_float2(re[p], im[p]);
+        }
+        out[((size_t)e * NCHI + f) * fstride + (size_t)(row0 + r) * pitch + sl] = val;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Strided pass (z or y): a CTA loads a tile of N rows x TX contiguous columns, transforms the
+// TX columns, stores the rows whose bins lie in the window.  Batches: blockIdx.x = tile +
+// n_tiles * lo, blockIdx.y = hi, with separate in/out strides (in float2 units).
+struct ColParams {
+    const float2 *in;
+    float2 *out;
+    int n_tiles;
+    long long in_row, out_row;        // stride between consecutive transform indices / slots
+    long long in_lo, out_lo;          // stride of the inner batch index (blockIdx.x / n_tiles)
+    long long in_hi, out_hi;          // stride of the outer batch index (blockIdx.y)
+    Window win;
+    const float2 *tw;
+};
+
+template <int LOGN> struct ColCfg {
+    static constexpr int N = 1 << LOGN;
+    static constexpr int TX = N >= 1024 ? 8 : (N >= 256 ? 16 : 32);
+    static constexpr int ELEMS = N * TX;
+    static constexpr int THREADS_RAW = ELEMS / 16;
+    static constexpr int THREADS = THREADS_RAW > 512 ? 512 : (THREADS_RAW < 64 ? 64 : THREADS_RAW);
+    static constexpr size_t SMEM = sizeof(float2) * ((size_t)ELEMS + N);
+};
+
+template <int LOGN>
+__global__ void __launch_bounds__(ColCfg<LOGN>::THREADS)
+k_colpass(const ColParams p)
+{
+    using Cfg = ColCfg<LOGN>;
+    constexpr int N = Cfg::N, TX = Cfg::TX, HX = TX / 2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *s = reinterpret_cast<float2 *>(smem_raw);
+    float2 *tw = s + Cfg::ELEMS;
+    const int tid = threadIdx.x;
+    const int tile = blockIdx.x % p.n_tiles, lo = blockIdx.x / p.n_tiles, hi = blockIdx.y;
+
+    const float2 *src = p.in + (size_t)hi * p.in_hi + (size_t)lo * p.in_lo + (size_t)tile * TX;
+#pragma unroll 4
+    for (int idx = tid; idx < N * HX; idx += Cfg::THREADS) {
+        const int i = idx / HX, c2 = idx % HX;
+        const float4 v = __ldcs(reinterpret_cast<const float4 *>(src + (size_t)i * p.in_row + 2 * c2));
+        *reinterpret_cast<float4 *>(s + i * TX + 2 * c2) = v;
+    }
+    for (int i = tid; i < N; i += Cfg::THREADS) tw[i] = p.tw[i];
+    __syncthreads();
+
+    ColAcc<N, TX> cacc{s};
+    fft_lines<LOGN, TX, Cfg::THREADS>(cacc, TX, tw, tid);
+
+    float2 *dst = p.out + (size_t)hi * p.out_hi + (size_t)lo * p.out_lo + (size_t)tile * TX;
+    for (int idx = tid; idx < p.win.W * HX; idx += Cfg::THREADS) {
+        const int sl = idx / HX, c2 = idx % HX;
+        const int b = (p.win.lo + sl) & (N - 1);
+        const float4 v = *reinterpret_cast<const float4 *>(s + b * TX + 2 * c2);
+        *reinterpret_cast<float4 *>(dst + (size_t)sl * p.out_row + 2 * c2) = v;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Ewald projection.  One thread per detector pixel and energy.
+struct EwaldParams {
+    int Nx, Ny, Nz, mode;
+    double dqx, dqy, dqz;
+    const double *k;            // [n_energy] wavenumbers, nm^-1
+    int e0;
+    Window wx, wy, wz;
+    int pitch;                  // x pitch of the spectrum cube
+    const float2 *spec;         // [e][f][slot_z][slot_y][pitch]
+    float4 *img;                // [e][Ny][Nx]  (I_xx, I_yy, I_xy, valid)
+};
+
+struct PixelGeom {
+    int n_nodes;
+    int node[2];
+    float wt[2];
+    float r[3];
+};
+
+// DESIGN 3-A5/A8/A11/A13; every double operation is individually rounded.
+__device__ __forceinline__ PixelGeom pixel_geometry(int ix, int iy, int Nx, int Ny, int Nz, int mode,
+                                                    double dqx, double dqy, double dqz, double k)
+{
+    PixelGeom g;
+    g.n_nodes = 0;
+    const double qx = __dmul_rn((double)(ix - Nx / 2), dqx);
+    const double qy = __dmul_rn((double)(iy - Ny / 2), dqy);
+    const double s2 = __dsub_rn(__dsub_rn(__dmul_rn(k, k), __dmul_rn(qx, qx)), __dmul_rn(qy, qy));
+    if (s2 < 0.0) return g;
+    const double root = __dsqrt_rn(s2);
+    const double qz = __dsub_rn(root, k);
+    g.r[0] = (float)__ddiv_rn(qx, k);
+    g.r[1] = (float)__ddiv_rn(qy, k);
+    g.r[2] = (float)__ddiv_rn(__dadd_rn(qz, k), k);
+    if (Nz == 1) { g.n_nodes = 1; g.node[0] = 0; g.wt[0] = 1.f; return g; }
+    const double gz = __ddiv_rn(qz, dqz);
+    if (mode == 0) {
+        const double n = floor(__dadd_rn(gz, 0.5));
+        if (n < (double)(-(Nz / 2))) return g;
+        g.n_nodes = 1; g.node[0] = (int)n; g.wt[0] = 1.f;
+        return g;
+    }
+    const double lo = floor(gz);
+    if (lo < (double)(-(Nz / 2))) return g;
+    const double t = __dsub_rn(gz, lo);
+    int c = 0;
+    if (__dsub_rn(1.0, t) > 0.0) { g.node[c] = (int)lo; g.wt[c] = (float)__dsub_rn(1.0, t); ++c; }
+    if (t > 0.0) { g.node[c] = (int)lo + 1; g.wt[c] = (float)t; ++c; }
+    g.n_nodes = c;
+    return g;
+}
+
+// (I - r r^T) applied to p~ for e = x (u) and e = y (v); returns |.|^2, |.|^2, Re<.,.>.
+__device__ __forceinline__ void project_pair(const float r[3], const float2 u[3], const float2 v[3],
+                                             float &sxx, float &syy, float &sxy)
+{
+    float2 ru = make_float2(r[0] * u[0].x + r[1] * u[1].x + r[2] * u[2].x, r[0] * u[0].y + r[1] * u[1].y + r[2] * u[2].y);
+    float2 rv = make_float2(r[0] * v[0].x + r[1] * v[1].x + r[2] * v[2].x, r[0] * v[0].y + r[1] * v[1].y + r[2] * v[2].y);
+    sxx = syy = sxy = 0.f;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const float2 wu = make_float2(u[d].x - r[d] * ru.x, u[d].y - r[d] * ru.y);
+        const float2 wv = make_float2(v[d].x - r[d] * rv.x, v[d].y - r[d] * rv.y);
+        sxx += wu.x * wu.x + wu.y * wu.y;
+        syy += wv.x * wv.x + wv.y * wv.y;
+        sxy += wu.x * wv.x + wu.y * wv.y;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_ewald_chi(const EwaldParams p)
+{
+    const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int iy = blockIdx.y * 8 + (threadIdx.x >> 5);
+    const int e = blockIdx.z;
+    if (ix >= p.Nx || iy >= p.Ny) return;
+    const double k = p.k[p.e0 + e];
+    const PixelGeom g = pixel_geometry(ix, iy, p.Nx, p.Ny, p.Nz, p.mode, p.dqx, p.dqy, p.dqz, k);
+    float axx = 0.f, ayy = 0.f, axy = 0.f;
+    bool valid = g.n_nodes > 0;
+    if (valid) {
+        const int sx = win_slot(p.wx, ix - p.Nx / 2), sy = win_slot(p.wy, iy - p.Ny / 2);
+        const size_t plane = (size_t)p.wy.W * p.pitch;
+        const size_t fstride = plane * p.wz.W;
+        const float2 *base = p.spec + (size_t)e * NCHI * fstride + (size_t)sy * p.pitch + sx;
+        const double k2 = k * k;
+        const float k4 = (float)(k2 * k2);
+        const bool inwin = sx < p.wx.W && sy < p.wy.W;
+        for (int j = 0; j < g.n_nodes; ++j) {
+            const int sz = win_slot(p.wz, g.node[j]);
+            float2 c[NCHI];
+#pragma unroll
+            for (int f = 0; f < NCHI; ++f)
+                c[f] = (inwin && sz < p.wz.W) ? __ldg(base + f * fstride + (size_t)sz * plane) : make_float2(0.f, 0.f);
+            const float2 u[3] = {c[0], c[1], c[2]}, v[3] = {c[1], c[3], c[4]};
+            float sxx, syy, sxy;
+            project_pair(g.r, u, v, sxx, syy, sxy);
+            const float w = g.wt[j] * k4;
+            axx = fmaf(w, sxx, axx); ayy = fmaf(w, syy, ayy); axy = fmaf(w, sxy, axy);
+        }
+    }
+    p.img[((size_t)e * p.Ny + iy) * p.Nx + ix] = make_float4(axx, ayy, axy, valid ? 1.f : 0.f);
+}
+
+// ------------------------------------------------------------------------------------------
+// Rotate back and average (DESIGN 3-A9/A10).  One thread per output pixel and energy; loops
+// over the angles.  cs[a] = (C, S) in double; csf[a] = (C^2, S^2, 2 C S) in float.
+struct RotateParams {
+    int Nx, Ny, n_angles;
+    const double2 *cs;
+    const float4 *csf;
+    const float4 *img;          // [e][Ny][Nx]
+    float *out;                 // [e][Ny][Nx]
+    unsigned int *counts;       // optional
+};
+
+__global__ void __launch_bounds__(256)
+k_rotate_avg(const RotateParams p)
+{
+    const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int iy = blockIdx.y * 8 + (threadIdx.x >> 5);
+    const int e = blockIdx.z;
+    if (ix >= p.Nx || iy >= p.Ny) return;
+    const float4 *img = p.img + (size_t)e * p.Ny * p.Nx;
+    const double rho = (double)p.Nx / (double)p.Ny;
+    const double u = (double)(ix - p.Nx / 2), v = (double)(iy - p.Ny / 2);
+    const double vr = v * rho, ur = u / rho;                 // exact: rho is a power of two
+    const double cx = (double)(p.Nx / 2), cy = (double)(p.Ny / 2);
+    float sum = 0.f;
+    unsigned int cnt = 0;
+    for (int a = 0; a < p.n_angles; ++a) {
+        const double2 cs = p.cs[a];
+        const double fx = __dadd_rn(__dsub_rn(__dmul_rn(cs.x, u), __dmul_rn(cs.y, vr)), cx);
+        const double fy = __dadd_rn(__dadd_rn(__dmul_rn(cs.y, ur), __dmul_rn(cs.x, v)), cy);
+        const double x0 = floor(fx), y0 = floor(fy);
+        const double al = fx - x0, be = fy - y0;
+        const int nx = al > 0.0 ? 2 : 1, ny = be > 0.0 ? 2 : 1;
+        if (x0 < 0.0 || y0 < 0.0 || x0 + (double)(nx - 1) > (double)(p.Nx - 1) || y0 + (double)(ny - 1) > (double)(p.Ny - 1))
+            continue;
+        const int X0 = (int)x0, Y0 = (int)y0;
+        const float4 w = p.csf[a];
+        const float fa = (float)al, fb = (float)be;
+        float acc = 0.f;
+        bool ok = true;
+        for (int jy = 0; jy < ny; ++jy)
+            for (int jx = 0; jx < nx; ++jx) {
+                const float4 t = __ldg(img + (size_t)(Y0 + jy) * p.Nx + (X0 + jx));
+                ok = ok && (t.w != 0.f);
+                const float I = w.x * t.x + w.y * t.y + w.z * t.z;
+                const float wt = (jx ? fa : 1.f - fa) * (jy ? fb : 1.f - fb);
+                acc = fmaf(wt, I, acc);
+            }
+        if (ok) { sum += acc; ++cnt; }
+    }
+    const size_t o = ((size_t)e * p.Ny + iy) * p.Nx + ix;
+    p.out[o] = cnt ? sum / (float)cnt : 0.f;
+    if (p.counts) p.counts[o] = cnt;
+}
+
+} // namespace cyr

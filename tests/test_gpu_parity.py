@@ -1,0 +1,147 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded
+inputs, element by element, with the north_star gates (tests/parity.py)."""
+import numpy as np
+import pytest
+
+from paper_2209_13121_b200 import workloads as W
+from tests.parity import compare, oracle_run
+
+pytestmark = pytest.mark.gpu
+
+ALGS = [1]      # binding.ALG_PER_ENERGY; SPECTRAL_BASIS is added when built
+
+
+def _gpu(w, alg, images=False):
+    from paper_2209_13121_b200 import binding
+    res = binding.simulate(w, algorithm=alg, want_counts=True, want_images=images)
+    out, cnt = res[0].cpu().numpy(), res[1].cpu().numpy()
+    if images:
+        return out, cnt, res[2].cpu().numpy(), res[-1]
+    return out, cnt, res[-1]
+
+
+@pytest.mark.parametrize("alg", ALGS)
+@pytest.mark.parametrize("mode", [W.EWALD_NEAREST, W.EWALD_TRILINEAR])
+@pytest.mark.parametrize("shape", [(8, 8, 4), (32, 16, 8), (16, 64, 2), (64, 32, 1), (4, 4, 16)])
+def test_tiny_random(shape, mode, alg):
+    nx, ny, nz = shape
+    w = W.tiny(seed=100 + nx + nz, nx=nx, ny=ny, nz=nz, n_mat=3, n_energy=3, voxel_nm=2.0, ewald=mode)
+    ref, rcnt = oracle_run(w)
+    out, cnt, _ = _gpu(w, alg)
+    compare(out, cnt, ref, rcnt, f"tiny{shape}")
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_stage_images_match_oracle_linear_images(alg):
+    w = W.tiny(seed=3, nx=32, ny=32, nz=16, n_mat=3, n_energy=2, voxel_nm=1.0, ewald=W.EWALD_TRILINEAR)
+    ref, rcnt, (Ixx, Iyy, Ixy, valid) = oracle_run(w, linear=True, return_images=True)
+    out, cnt, imgs, ctx = _gpu(w, alg, images=True)
+    assert imgs.shape[0] == 2
+    for e in range(2):
+        assert (imgs[e, :, :, 3].astype(bool) == valid[e].astype(bool)).all()
+        for j, r in enumerate((Ixx[e], Iyy[e], Ixy[e])):
+            err = np.abs(imgs[e, :, :, j] - r).max() / np.abs(Ixx[e]).max()
+            assert err < 5e-6, (e, j, err)
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_cfg1_full(alg):
+    w = W.cfg1()
+    ref, rcnt = oracle_run(w)
+    out, cnt, _ = _gpu(w, alg)
+    r = compare(out, cnt, ref, rcnt, "cfg1")
+    print("cfg1", r)
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_cfg2_reduced_definition_mode(alg):
+    w = W.cfg2(n=64, n_energy=3)
+    ref, rcnt = oracle_run(w)
+    out, cnt, _ = _gpu(w, alg)
+    print("cfg2/64", compare(out, cnt, ref, rcnt, "cfg2/64"))
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_cfg2_full_size(alg):
+    """BASELINE configs[1] at full size (the bench workload), oracle in linear mode."""
+    w = W.cfg2()
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, ctx = _gpu(w, alg)
+    print("cfg2", compare(out, cnt, ref, rcnt, "cfg2"), ctx.stats())
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_cfg3_reduced(alg):
+    w = W.cfg3(nx=64, ny=64, nz=32, n_energy=4, grain=8.0)
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, _ = _gpu(w, alg)
+    print("cfg3/64", compare(out, cnt, ref, rcnt, "cfg3/64"))
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_cfg4_reduced(alg):
+    w = W.cfg4(n=256, n_energy=3)
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, _ = _gpu(w, alg)
+    print("cfg4/256", compare(out, cnt, ref, rcnt, "cfg4/256"))
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_edge_cases(alg):
+    # single angle, 90 degrees (pixel permutation), all-isotropic materials, Nz = 2
+    w = W.tiny(seed=9, nx=16, ny=16, nz=2, n_mat=2, n_energy=1, voxel_nm=3.0, ewald=W.EWALD_TRILINEAR,
+               angles=(90.0, 0.0, 90.0))
+    ref, rcnt = oracle_run(w)
+    out, cnt, _ = _gpu(w, alg)
+    compare(out, cnt, ref, rcnt, "single-angle-90")
+    iso = [(m[0], None, None, None) for m in w.materials]
+    w2 = W.Workload("iso", w.Nx, w.Ny, w.Nz, w.voxel_nm, iso, w.energies, w.delta_par, w.beta_par, w.delta_par,
+                    w.beta_par, (0.0, 45.0, 315.0), W.EWALD_NEAREST)
+    ref, rcnt = oracle_run(w2)
+    out, cnt, _ = _gpu(w2, alg)
+    compare(out, cnt, ref, rcnt, "all-isotropic")
+    # a detector mostly off the Ewald sphere: tiny voxels -> large dq, few valid pixels
+    w3 = W.tiny(seed=10, nx=32, ny=32, nz=8, n_mat=2, n_energy=2, voxel_nm=0.4, ewald=W.EWALD_NEAREST)
+    ref, rcnt = oracle_run(w3)
+    assert (rcnt == 0).mean() > 0.5
+    out, cnt, _ = _gpu(w3, alg)
+    compare(out, cnt, ref, rcnt, "mostly-invalid")
+
+
+def test_errors_and_not_ready():
+    import torch
+    from paper_2209_13121_b200 import binding
+    ctx = binding.Context(16, 16, 4, 1, 2.0)
+    out = torch.empty((1, 16, 16), device="cuda")
+    with pytest.raises(binding.CyrsoxsError) as ei:
+        ctx.run(out.data_ptr())
+    assert ei.value.status == binding.ERR_NOT_READY
+    for bad in [(0.0, 0.0, 10.0), (10.0, 5.0, 0.0)]:
+        with pytest.raises(binding.CyrsoxsError) as ei:
+            ctx.set_angles(*bad)
+        assert ei.value.status == binding.ERR_INVALID_ARG
+    with pytest.raises(binding.CyrsoxsError):
+        ctx.set_ewald(7)
+    with pytest.raises(binding.CyrsoxsError):
+        ctx.set_optical_constants([-1.0], [[0]], [[0]], [[0]], [[0]])
+    phi = torch.ones((4, 16, 16), device="cuda")
+    with pytest.raises(binding.CyrsoxsError):
+        ctx.set_morphology([(phi, phi, None, None)])      # S without theta/psi
+    ctx.close()
+
+
+def test_host_output_and_host_morphology():
+    """End-to-end entry: morphology from host arrays, images written to pinned host memory."""
+    import torch
+    from paper_2209_13121_b200 import binding
+    w = W.tiny(seed=12, nx=32, ny=32, nz=8, n_mat=2, n_energy=5, voxel_nm=2.0)
+    ref, rcnt = oracle_run(w)
+    ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    s = torch.cuda.current_stream().cuda_stream
+    ctx.set_morphology_host(w.materials, s)
+    ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald); ctx.set_algorithm(ALGS[0])
+    out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32).pin_memory()
+    ctx.run(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    compare(out.numpy(), None, ref, rcnt, "host-io")
