@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the CyRSoXS hot path on B200 (contract: task prompt section 4).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2]
+
+A "step" is one pass of the whole hot path (all energies x all E-field angles of the
+workload) over one synthetic morphology.  Metric: E-angle patterns/s (BASELINE.json), device
+timed with CUDA events on the launching stream; voxel.angle evaluations/s is reported beside
+it.  The default workload is BASELINE.json configs[1] (3-D cube 128^3, 10 energies x 36
+angles).  N > 1: energies are independent units, so every rank simulates its
+own slice of a N-times longer energy list on the same morphology -- no data-path collective,
+weak scaling.  `--impl reference` times the CPU oracle (as it stands) on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2209_13121_b200 import workloads as W  # noqa: E402
+
+METRIC = "E-angle patterns/s (device-timed)"
+UNIT = "patterns/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def make_workload(name: str, rank: int, world: int):
+    if name == "cfg1":
+        w = W.cfg1()
+    elif name == "cfg2":
+        w = W.cfg2()
+    elif name == "cfg3":
+        w = W.cfg3()
+    elif name == "cfg4":
+        w = W.cfg4()
+    elif name == "cfg5":
+        w = W.cfg5()
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    if world > 1:
+        # weak scaling: a world-times longer energy list over the same range, rank r owns slice r
+        E = np.linspace(w.energies[0], w.energies[-1], w.n_energy * world) if w.n_energy > 1 else np.repeat(w.energies, world)
+        tabs = []
+        for t in (w.delta_par, w.beta_par, w.delta_perp, w.beta_perp):
+            full = np.stack([np.interp(E, w.energies, t[:, m]) if w.n_energy > 1 else np.repeat(t[:, m], world)
+                             for m in range(w.n_mat)], 1).astype(np.float32)
+            tabs.append(full[rank * w.n_energy:(rank + 1) * w.n_energy])
+        w.energies = E[rank * w.n_energy:(rank + 1) * w.n_energy].copy()
+        w.delta_par, w.beta_par, w.delta_perp, w.beta_perp = tabs
+    return w
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                o = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                   capture_output=True, text=True, timeout=5).stdout.strip()
+                if o:
+                    self.rows.append([x.strip() for x in o.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for j, n in enumerate(names) if any(r[3 + j].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
+                "samples": len(sm), "power_w_max": max(float(r[2]) for r in self.rows)}
+
+
+def oracle_sample(w, budget_s: float = 20.0):
+    """The oracle as it stands (definition mode) on a bounded sample: one energy, as many of
+    the workload's angles as fit the budget (at least one)."""
+    import oracle
+    t0 = time.perf_counter()
+    oracle.run(w.materials, w.voxel_nm, w.energies[:1], w.delta_par[:1], w.beta_par[:1], w.delta_perp[:1], w.beta_perp[:1],
+               (w.angles[0], w.angles[1], w.angles[0]), w.ewald)
+    t1 = time.perf_counter() - t0
+    n = int(max(1, min(w.n_angles, budget_s / max(t1, 1e-9))))
+    t0 = time.perf_counter()
+    oracle.run(w.materials, w.voxel_nm, w.energies[:1], w.delta_par[:1], w.beta_par[:1], w.delta_perp[:1], w.beta_perp[:1],
+               (w.angles[0], w.angles[1], w.angles[0] + (n - 1) * w.angles[1]), w.ewald)
+    dt = time.perf_counter() - t0
+    return n / dt, n, dt, oracle.num_threads()
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    w = make_workload(args.workload, 0, 1)
+    vals = []
+    for i in range(args.warmup + args.steps):
+        v, n, dt, cores = oracle_sample(w, budget_s=max(2.0, 60.0 / (args.warmup + args.steps)))
+        if i >= args.warmup:
+            vals.append((v, n, dt))
+    value = sum(v[1] for v in vals) / sum(v[2] for v in vals)
+    sample = f"1 energy x {vals[0][1]} of {w.n_angles} angles per step, definition mode (polarization, 3 FFTs, Ewald, rotate per angle)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sum(v[2] for v in vals) / len(vals), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{w.name}: {w.Nx}x{w.Ny}x{w.Nz}, {w.n_mat} materials, {w.n_energy} energies x {w.n_angles} angles",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2209_13121_b200 import binding, build
+    build.build()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = make_workload(args.workload, rank, world)
+    alg = {"auto": binding.ALG_AUTO, "per_energy": binding.ALG_PER_ENERGY, "spectral": binding.ALG_SPECTRAL_BASIS}[args.alg]
+    mats = [tuple(None if a is None else torch.from_numpy(a).to(dev) for a in m) for m in w.materials]
+    ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    ctx.set_morphology(mats)
+    ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald); ctx.set_algorithm(alg)
+    out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    sptr = stream.cuda_stream
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def one_step():
+        flush.fill_(1)                                  # L2 flush between timed iterations (outside the events)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        ctx.run(out.data_ptr(), sptr)
+        b.record(stream)
+        return a, b
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    evs = [one_step() for _ in range(args.steps)]
+    barrier()
+    sampler.stop_flag = True
+    sampler.join(timeout=3)
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    st = ctx.stats()
+    launches = st["kernel_launches"] * args.steps
+
+    # ---- end to end through the C ABI with host buffers (H2D + D2H inside the timed region)
+    pinned = [tuple(None if a is None else torch.from_numpy(a).pin_memory() for a in m) for m in w.materials]
+    h_out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32).pin_memory()
+    ctx2 = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    ctx2.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    ctx2.set_angles(*w.angles); ctx2.set_ewald(w.ewald); ctx2.set_algorithm(alg)
+    h2d = sum(a.numel() * 4 for m in pinned for a in m if a is not None)
+    d2h = h_out.numel() * 4
+
+    def e2e_step():
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        ctx2.set_morphology_host(pinned, sptr)
+        ctx2.run(h_out.data_ptr(), sptr)
+        b.record(stream)
+        return a, b
+
+    for _ in range(max(1, min(args.warmup, 3))):
+        e2e_step()
+    barrier()
+    n_e2e = max(1, min(args.steps, 5))
+    ev2 = [e2e_step() for _ in range(n_e2e)]
+    barrier()
+    e2e_ms = float(sum(a.elapsed_time(b) for a, b in ev2)) / n_e2e
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+
+    # ---- per-stage device times (CUDA events on the run's stream, inside the library) for the roofline
+    ctx.set_profiling(True)
+    stage_ms = {k: 0.0 for k in binding.STAGES}
+    nprof = max(1, min(args.steps, 5))
+    for _ in range(nprof):
+        flush.fill_(1)
+        ctx.run(out.data_ptr(), sptr)
+        s2 = ctx.stats()
+        for k in stage_ms:
+            stage_ms[k] += s2["stage_ms"][k]
+    ctx.set_profiling(False)
+    dom = max(stage_ms, key=lambda k: stage_ms[k])
+    peak, peak_src = load_peaks()
+    dom_launches = max(1, st["stage_launches"][dom])
+    dom_ms_per_launch = stage_ms[dom] / nprof / dom_launches
+    dom_bytes_per_launch = st["stage_bytes"][dom] / dom_launches
+    achieved = dom_bytes_per_launch / (dom_ms_per_launch * 1e-3) / 1e9 if dom_ms_per_launch > 0 else 0.0
+    whole_bytes = sum(st["stage_bytes"].values())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    patterns = w.n_energy * w.n_angles * world * args.steps
+    value = patterns / (total_ms * 1e-3)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {
+            "workload": f"{w.name}: {w.Nx}x{w.Ny}x{w.Nz} voxels, {w.n_mat} materials, {w.n_energy} energies x "
+                        f"{w.n_angles} angles per GPU, ewald={'trilinear' if w.ewald else 'nearest'} (BASELINE.json configs[1])"
+                        if args.workload == "cfg2" else f"{w.name}: {w.Nx}x{w.Ny}x{w.Nz}, {w.n_mat} materials, "
+                        f"{w.n_energy} energies x {w.n_angles} angles per GPU",
+            "algorithm": {1: "per_energy", 2: "spectral_basis"}.get(st["algorithm"], "?"),
+            "energy_batch": st["energy_batch"], "l2": "flushed between timed steps (256 MB write)",
+            "parallelism": f"energies sharded over {world} GPU(s), no collective",
+        },
+        "voxel_angle_evals_per_s": value * w.n_vox,
+        "e2e": {"value": w.n_energy * w.n_angles * world / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms},
+        "gpu_launches": int(launches),
+        "clocks": sampler.summary(),
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "bytes_per_launch": dom_bytes_per_launch, "ms_per_launch": dom_ms_per_launch,
+                     "stage_ms_per_step": {k: v / nprof for k, v in stage_ms.items()},
+                     "stage_gbs": {k: (st["stage_bytes"][k] / (stage_ms[k] / nprof * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0)
+                                   for k in stage_ms},
+                     "whole_step": {"bytes": whole_bytes, "achieved": whole_bytes / (total_ms / args.steps * 1e-3) / 1e9,
+                                    "frac": whole_bytes / (total_ms / args.steps * 1e-3) / 1e9 / peak}},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        v, n, dt, cores = oracle_sample(w, budget_s=20.0)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"1 energy x {n} of {w.n_angles} angles of the same workload, definition mode, {dt:.1f} s"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--alg", default="auto", choices=["auto", "per_energy", "spectral"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world == 1 and args.gpus > 1 and args.impl == "ours":
+        # launched without torchrun: re-exec under torch.distributed.run on this node
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", "29531", os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
