@@ -87,7 +87,7 @@ typedef struct {
 
 /* Creates a context for an Nx x Ny x Nz voxel model with n_mat materials and cubic voxels of
  * edge voxel_nm ("voxels are considered perfect cubes").  Sizes must be powers of two,
- * 1 <= Nz, 2 <= Nx, Ny <= 4096, Nz <= 4096, 1 <= n_mat <= 32, voxel_nm > 0 (else
+ * 4 <= Nx <= 2048, 2 <= Ny <= 2048, 1 <= Nz <= 2048, 1 <= n_mat <= 32, voxel_nm > 0 (else
  * INVALID_ARG).  Uses the current CUDA device.  *out is NULL on failure. */
 cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm, cyrsoxs_ctx **out);
 

@@ -55,9 +55,15 @@ struct cyrsoxs_ctx {
     int alg = CYRSOXS_ALG_AUTO;
     int profiling = 0;
     unsigned int *d_counts = nullptr;
+    // SPECTRAL_BASIS plan (rebuilt per run from the morphology's NULL pattern and the optics)
+    BasisGroups groups{};
+    int n_pack = 0;
+    std::vector<int> basis_kind, basis_mat;     // [2 n_pack]
+    DevBuf d_bcoef, d_bkind;
+    bool plan_dirty = true;
+    unsigned long long null_pattern = ~0ull;
     // workspace
     DevBuf A1, A2, A3, img, twx, twy, twz, stage_out[2];
-    void *pinned_probe = nullptr;
     // last run
     cyrsoxs_stats stats{};
     cudaStream_t last_stream = nullptr;
@@ -158,13 +164,13 @@ struct Plan {
 
 // Windows from the largest wavenumber in [e0, e1): valid pixels have |q_x|, |q_y| <= k and
 // k_z nodes in [-(k/dq_z) - 1, 0] (Eq. 8).  One extra bin of slack on every side.
-void windows_for(const cyrsoxs_ctx *c, double kmax, Window &wx, Window &wy, Window &wz, int &pitch)
+void windows_for(const cyrsoxs_ctx *c, double kmax, Window &wx, Window &wy, Window &wz, int &pitch, bool sym_z = false)
 {
     int Kx = (int)floor(kmax / c->dqx) + 1, Ky = (int)floor(kmax / c->dqy) + 1;
     wx = make_window(c->Nx, Kx, true);
     wy = make_window(c->Ny, Ky, true);
     if (c->Nz == 1) { wz.N = 1; wz.lo = 0; wz.W = 1; }
-    else { int Kz = (int)floor(kmax / c->dqz) + 2; wz = make_window(c->Nz, Kz, false); }
+    else { int Kz = (int)floor(kmax / c->dqz) + 2; wz = make_window(c->Nz, Kz, sym_z); }
     pitch = round_up(wx.W, 32);
 }
 
@@ -322,6 +328,163 @@ cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int
     return CYRSOXS_OK;
 }
 
+template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, const BasisGroups &g, float2 *out,
+                                                   const Window &wx, int pitch)
+{
+    using Cfg = XBasisCfg<LOGN>;
+    static bool attr_done[64] = {false};
+    if (!attr_done[c->device & 63]) {
+        CUDA_TRY(c, cudaFuncSetAttribute(k_xpass_basis<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        attr_done[c->device & 63] = true;
+    }
+    const int rows = c->Ny * c->Nz;
+    dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS, g.n_groups);
+    k_xpass_basis<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(c->mp, g, out, rows, wx, pitch, (const float2 *)c->twx.p);
+    CUDA_TRY(c, cudaGetLastError());
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, const BasisGroups &g, float2 *out, const Window &wx, int pitch)
+{
+    switch (ilog2(c->Nx)) {
+#define CASE(L) case L: return launch_xbasis_t<L>(c, st, g, out, wx, pitch);
+        CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11)
+#undef CASE
+    }
+    return fail(c, CYRSOXS_ERR_INVALID_ARG, "unsupported Nx");
+}
+
+// Groups of materials with at most BASIS_MAX_FIELDS real basis fields each (7 per aligned, 1 per
+// isotropic material), every group padded to whole packs.  Also the per-field kind/material
+// tables and the per-energy complex coefficient of each field (times 1/2 for the unpacking).
+cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c)
+{
+    BasisGroups &G = c->groups;
+    memset(&G, 0, sizeof G);
+    c->basis_kind.clear(); c->basis_mat.clear();
+    int pack = 0;
+    BasisGroup cur{};
+    cur.pack0 = 0;
+    auto flush = [&]() {
+        if (cur.n_mat == 0) return true;
+        if (G.n_groups >= BASIS_MAX_GROUPS) return false;
+        if (cur.n_fields & 1) { c->basis_kind.push_back(BK_NONE); c->basis_mat.push_back(0); }
+        pack += (cur.n_fields + 1) / 2;
+        G.g[G.n_groups++] = cur;
+        cur = BasisGroup{};
+        cur.pack0 = pack;
+        return true;
+    };
+    for (int m = 0; m < c->n_mat; ++m) {
+        const bool aligned = c->mp.S[m] != nullptr;
+        const int nf = aligned ? 7 : 1;
+        if (cur.n_fields + nf > BASIS_MAX_FIELDS && !flush()) return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "too many basis groups");
+        cur.mat[cur.n_mat++] = m;
+        cur.n_fields += nf;
+        if (aligned) for (int kd = BK_PHI; kd <= BK_YZ; ++kd) { c->basis_kind.push_back(kd); c->basis_mat.push_back(m); }
+        else { c->basis_kind.push_back(BK_PHI); c->basis_mat.push_back(m); }
+    }
+    if (!flush()) return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "too many basis groups");
+    c->n_pack = pack;
+    const int nb = 2 * pack;
+    std::vector<float2> coef((size_t)c->nE * nb);
+    for (int e = 0; e < c->nE; ++e)
+        for (int b = 0; b < nb; ++b) {
+            const float *o = &c->coef[((size_t)e * c->n_mat + c->basis_mat[b]) * 6];
+            float2 v = make_float2(0.f, 0.f);
+            switch (c->basis_kind[b]) {
+            case BK_PHI: v = make_float2(o[0], o[1]); break;
+            case BK_W: v = make_float2(o[2], o[3]); break;
+            case BK_NONE: break;
+            default: v = make_float2(o[4], o[5]); break;
+            }
+            coef[(size_t)e * nb + b] = make_float2(0.5f * v.x, 0.5f * v.y);
+        }
+    cyrsoxs_status s;
+    if ((s = ensure(c, c->d_bcoef, sizeof(float2) * coef.size())) != CYRSOXS_OK) return s;
+    if ((s = ensure(c, c->d_bkind, sizeof(int) * nb)) != CYRSOXS_OK) return s;
+    CUDA_TRY(c, cudaMemcpy(c->d_bcoef.p, coef.data(), sizeof(float2) * coef.size(), cudaMemcpyHostToDevice));
+    CUDA_TRY(c, cudaMemcpy(c->d_bkind.p, c->basis_kind.data(), sizeof(int) * nb, cudaMemcpyHostToDevice));
+    c->plan_dirty = false;
+    return CYRSOXS_OK;
+}
+
+// Spectra of all basis packs: x -> z -> y, once per run.  A3 = [pack][wz][wy][pitch].
+cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &wx, const Window &wy, const Window &wz, int pitch)
+{
+    const BasisGroups &G = c->groups;
+    const size_t rows = (size_t)c->Ny * c->Nz;
+    const int F = c->n_pack;
+    float2 *A1 = (float2 *)c->A1.p, *A2 = (float2 *)c->A2.p, *A3 = (float2 *)c->A3.p;
+    const double nvox = (double)c->Nx * c->Ny * c->Nz;
+    cyrsoxs_status s;
+    {
+        StageTimer t(c, st, CYRSOXS_STAGE_XPASS);
+        if ((s = launch_xbasis(c, st, G, A1, wx, pitch)) != CYRSOXS_OK) return s;
+        double n_iso = 0, n_al = 0;
+        for (int m = 0; m < c->n_mat; ++m) (c->mp.S[m] ? n_al : n_iso) += 1;
+        c->stats.stage_bytes[CYRSOXS_STAGE_XPASS] += nvox * (16.0 * n_al + 4.0 * n_iso) + 8.0 * F * rows * pitch;
+    }
+    const float2 *ysrc = A1;
+    if (c->Nz > 1) {
+        StageTimer t(c, st, CYRSOXS_STAGE_ZPASS);
+        ColParams p{};
+        p.in = A1; p.out = A2;
+        p.in_row = (long long)c->Ny * pitch; p.out_row = (long long)c->Ny * pitch;
+        p.in_lo = pitch; p.out_lo = pitch;
+        p.in_hi = (long long)c->Nz * c->Ny * pitch; p.out_hi = (long long)wz.W * c->Ny * pitch;
+        p.win = wz; p.tw = (const float2 *)c->twz.p;
+        if ((s = launch_colpass(c, st, c->Nz, p, c->Ny, F, pitch)) != CYRSOXS_OK) return s;
+        c->stats.stage_bytes[CYRSOXS_STAGE_ZPASS] += 8.0 * F * c->Ny * pitch * ((double)c->Nz + wz.W);
+        ysrc = A2;
+    }
+    {
+        StageTimer t(c, st, CYRSOXS_STAGE_YPASS);
+        ColParams p{};
+        p.in = ysrc; p.out = A3;
+        p.in_row = pitch; p.out_row = pitch;
+        p.in_lo = (long long)c->Ny * pitch; p.out_lo = (long long)wy.W * pitch;
+        p.in_hi = (long long)wz.W * c->Ny * pitch; p.out_hi = (long long)wz.W * wy.W * pitch;
+        p.win = wy; p.tw = (const float2 *)c->twy.p;
+        if ((s = launch_colpass(c, st, c->Ny, p, wz.W, F, pitch)) != CYRSOXS_OK) return s;
+        c->stats.stage_bytes[CYRSOXS_STAGE_YPASS] += 8.0 * F * wz.W * pitch * ((double)c->Ny + wy.W);
+    }
+    return CYRSOXS_OK;
+}
+
+// One energy batch of SPECTRAL_BASIS: shell gather + rotate.
+cyrsoxs_status run_batch_spectral(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, const Window &wx, const Window &wy,
+                                  const Window &wz, int pitch, float *d_out, unsigned int *d_cnt)
+{
+    dim3 g2((c->Nx + 31) / 32, (c->Ny + 7) / 8, eb);
+    {
+        StageTimer t(c, st, CYRSOXS_STAGE_EWALD);
+        EwaldBasisParams q{};
+        EwaldParams &p = q.g;
+        p.Nx = c->Nx; p.Ny = c->Ny; p.Nz = c->Nz; p.mode = c->ewald;
+        p.dqx = c->dqx; p.dqy = c->dqy; p.dqz = c->dqz;
+        p.k = (const double *)c->d_k.p; p.e0 = e0;
+        p.wx = wx; p.wy = wy; p.wz = wz; p.pitch = pitch;
+        p.spec = (const float2 *)c->A3.p; p.img = (float4 *)c->img.p;
+        q.n_pack = c->n_pack; q.coef = (const float2 *)c->d_bcoef.p; q.kind = (const int *)c->d_bkind.p;
+        k_ewald_basis<<<g2, 256, 0, st>>>(q);
+        CUDA_TRY(c, cudaGetLastError());
+        const double nodes = (c->Nz > 1 && c->ewald == CYRSOXS_EWALD_TRILINEAR) ? 2.0 : 1.0;
+        c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * 0.785 * nodes * 2.0 * c->n_pack * 8.0 + 16.0 * c->Nx * c->Ny);
+    }
+    {
+        StageTimer t(c, st, CYRSOXS_STAGE_ROTATE);
+        RotateParams p{};
+        p.Nx = c->Nx; p.Ny = c->Ny; p.n_angles = c->nA;
+        p.cs = (const double2 *)c->d_cs.p; p.csf = (const float4 *)c->d_csf.p;
+        p.img = (const float4 *)c->img.p; p.out = d_out; p.counts = d_cnt;
+        k_rotate_avg<<<g2, 256, 0, st>>>(p);
+        CUDA_TRY(c, cudaGetLastError());
+        c->stats.stage_bytes[CYRSOXS_STAGE_ROTATE] += eb * (20.0 * c->Nx * c->Ny);
+    }
+    return CYRSOXS_OK;
+}
+
 } // namespace
 
 // =========================================================================================
@@ -365,7 +528,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
     clear_prof(c);
     for (void *p : c->owned_morph) cudaFree(p);
     for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_cs, &c->d_csf, &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
-                      &c->stage_out[0], &c->stage_out[1]})
+                      &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind})
         release(*b);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     for (int i = 0; i < 2; ++i) {
@@ -373,6 +536,13 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
         if (c->ev_copy[i]) cudaEventDestroy(c->ev_copy[i]);
     }
     delete c;
+}
+
+static void note_null_pattern(cyrsoxs_ctx *c)
+{
+    unsigned long long pat = 0;
+    for (int m = 0; m < c->n_mat; ++m) pat |= (unsigned long long)(c->mp.S[m] != nullptr) << m;
+    if (pat != c->null_pattern) { c->null_pattern = pat; c->plan_dirty = true; }
 }
 
 static cyrsoxs_status check_morph_tables(cyrsoxs_ctx *c, const float *const *phi, const float *const *S,
@@ -405,6 +575,7 @@ cyrsoxs_status cyrsoxs_set_morphology(cyrsoxs_ctx *c, const float *const *d_phi,
         c->mp.theta[m] = d_theta ? d_theta[m] : nullptr;
         c->mp.psi[m] = d_psi ? d_psi[m] : nullptr;
     }
+    note_null_pattern(c);
     c->have_morph = true;
     return CYRSOXS_OK;
 }
@@ -456,6 +627,7 @@ cyrsoxs_status cyrsoxs_set_morphology_host(cyrsoxs_ctx *c, const float *const *h
         c->mp.phi[m] = dptr[4 * m]; c->mp.S[m] = dptr[4 * m + 1];
         c->mp.theta[m] = dptr[4 * m + 2]; c->mp.psi[m] = dptr[4 * m + 3];
     }
+    note_null_pattern(c);
     c->have_morph = true;
     return CYRSOXS_OK;
 }
@@ -502,6 +674,7 @@ cyrsoxs_status cyrsoxs_set_optical_constants(cyrsoxs_ctx *c, int n_energy, const
     CUDA_TRY(c, cudaMemcpy(c->d_coef.p, c->coef.data(), sizeof(float) * c->coef.size(), cudaMemcpyHostToDevice));
     CUDA_TRY(c, cudaMemcpy(c->d_k.p, c->k.data(), sizeof(double) * n_energy, cudaMemcpyHostToDevice));
     c->have_optics = true;
+    c->plan_dirty = true;
     return CYRSOXS_OK;
 }
 
@@ -580,7 +753,6 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     if (!c->have_morph || !c->have_optics || !c->have_angles)
         return fail(c, CYRSOXS_ERR_NOT_READY, "run needs morphology, optical constants and angles (missing:%s%s%s)",
                     c->have_morph ? "" : " morphology", c->have_optics ? "" : " optical-constants", c->have_angles ? "" : " angles");
-    if (c->alg == CYRSOXS_ALG_SPECTRAL_BASIS) return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "SPECTRAL_BASIS is not built yet");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
 
@@ -592,28 +764,45 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     if (pa.type != cudaMemoryTypeHost && pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
         return fail(c, CYRSOXS_ERR_INVALID_ARG, "out must be device memory or pinned host memory");
 
+    cyrsoxs_status s;
+    if (c->plan_dirty && (s = build_basis_plan(c)) != CYRSOXS_OK) return s;
+    // AUTO: the basis needs n_pack complex transforms per run, PER_ENERGY 5 per energy
+    int alg = c->alg;
+    if (alg == CYRSOXS_ALG_AUTO) alg = (NCHI * c->nE > c->n_pack) ? CYRSOXS_ALG_SPECTRAL_BASIS : CYRSOXS_ALG_PER_ENERGY;
+    const bool spectral = alg == CYRSOXS_ALG_SPECTRAL_BASIS;
+
     // plan: windows for the largest k, energy batch from the free memory
     double kmax = *std::max_element(c->k.begin(), c->k.end());
     Window wx, wy, wz;
     int pitch;
-    windows_for(c, kmax, wx, wy, wz, pitch);
+    windows_for(c, kmax, wx, wy, wz, pitch, spectral);
     const size_t npix = (size_t)c->Nx * c->Ny;
-    const size_t a1 = (size_t)NCHI * c->Nz * c->Ny * pitch, a2 = c->Nz > 1 ? (size_t)NCHI * wz.W * c->Ny * pitch : 0,
-                 a3 = (size_t)NCHI * wz.W * wy.W * pitch;
-    const size_t per_e = sizeof(float2) * (a1 + a2 + a3) + sizeof(float4) * npix + (out_on_host ? 2 * sizeof(float) * npix : 0);
+    const size_t F1 = spectral ? (size_t)c->n_pack : (size_t)NCHI;
+    const size_t a1 = F1 * c->Nz * c->Ny * pitch, a2 = c->Nz > 1 ? F1 * wz.W * c->Ny * pitch : 0, a3 = F1 * wz.W * wy.W * pitch;
+    const size_t per_img = sizeof(float4) * npix + (out_on_host ? 2 * sizeof(float) * npix : 0);
+    const size_t per_e = spectral ? per_img : sizeof(float2) * (a1 + a2 + a3) + per_img;
+    const size_t fixed = spectral ? sizeof(float2) * (a1 + a2 + a3) : 0;
     size_t free_b = 0, total_b = 0;
     CUDA_TRY(c, cudaMemGetInfo(&free_b, &total_b));
     const size_t have = c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap;
     const size_t budget = (size_t)((double)(free_b + have) * 0.85);
-    int eb = (int)std::min<size_t>((size_t)c->nE, std::max<size_t>(1, budget / per_e));
-    // keep batches small enough that several fit in flight and large enough to fill the GPU
-    const size_t target = (size_t)1 << 31;        // ~2 GiB of fields per batch is plenty of parallelism
-    eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / (sizeof(float2) * a1))));
-    eb = std::min(eb, 64);
-    cyrsoxs_status s;
-    if ((s = ensure(c, c->A1, sizeof(float2) * a1 * eb)) != CYRSOXS_OK) return s;
-    if (a2 && (s = ensure(c, c->A2, sizeof(float2) * a2 * eb)) != CYRSOXS_OK) return s;
-    if ((s = ensure(c, c->A3, sizeof(float2) * a3 * eb)) != CYRSOXS_OK) return s;
+    if (fixed + per_e > budget)
+        return fail(c, CYRSOXS_ERR_OOM, "workspace of %.1f GB does not fit in %.1f GB of free device memory",
+                    (double)(fixed + per_e) / 1e9, (double)budget / 1e9);
+    int eb = (int)std::min<size_t>((size_t)c->nE, std::max<size_t>(1, (budget - fixed) / per_e));
+    if (!spectral) {
+        // ~2 GiB of fields per batch is plenty of parallelism
+        const size_t target = (size_t)1 << 31;
+        eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / (sizeof(float2) * a1))));
+    } else {
+        const size_t target = (size_t)1 << 32;
+        eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / per_img)));
+    }
+    eb = std::min(eb, 256);
+    const size_t mult = spectral ? 1 : (size_t)eb;
+    if ((s = ensure(c, c->A1, sizeof(float2) * a1 * mult)) != CYRSOXS_OK) return s;
+    if (a2 && (s = ensure(c, c->A2, sizeof(float2) * a2 * mult)) != CYRSOXS_OK) return s;
+    if ((s = ensure(c, c->A3, sizeof(float2) * a3 * mult)) != CYRSOXS_OK) return s;
     if ((s = ensure(c, c->img, sizeof(float4) * npix * eb)) != CYRSOXS_OK) return s;
     if (out_on_host) {
         for (int i = 0; i < 2; ++i)
@@ -627,26 +816,30 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
 
     clear_prof(c);
     memset(&c->stats, 0, sizeof c->stats);
-    c->stats.algorithm = CYRSOXS_ALG_PER_ENERGY;
+    c->stats.algorithm = alg;
     c->stats.n_energy = c->nE; c->stats.n_angles = c->nA; c->stats.energy_batch = eb;
     c->stats.workspace_bytes = (double)(c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap);
     c->last_stream = st;
+
+    if (spectral && (s = run_basis_spectra(c, st, wx, wy, wz, pitch)) != CYRSOXS_OK) return s;
 
     int nb = 0;
     for (int e0 = 0; e0 < c->nE; e0 += eb, ++nb) {
         const int n = std::min(eb, c->nE - e0);
         unsigned int *cnt = c->d_counts ? c->d_counts + (size_t)e0 * npix : nullptr;
-        if (!out_on_host) {
-            if ((s = run_batch_per_energy(c, st, e0, n, out + (size_t)e0 * npix, cnt)) != CYRSOXS_OK) return s;
-        } else {
-            const int slot = nb & 1;
+        float *dst = out + (size_t)e0 * npix;
+        const int slot = nb & 1;
+        if (out_on_host) {
             // the staging slot is free once the copy issued two batches ago has finished
             if (nb >= 2) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_copy[slot], 0));
-            if ((s = run_batch_per_energy(c, st, e0, n, (float *)c->stage_out[slot].p, cnt)) != CYRSOXS_OK) return s;
+            dst = (float *)c->stage_out[slot].p;
+        }
+        s = spectral ? run_batch_spectral(c, st, e0, n, wx, wy, wz, pitch, dst, cnt) : run_batch_per_energy(c, st, e0, n, dst, cnt);
+        if (s != CYRSOXS_OK) return s;
+        if (out_on_host) {
             CUDA_TRY(c, cudaEventRecord(c->ev_batch[slot], st));
             CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_batch[slot], 0));
-            CUDA_TRY(c, cudaMemcpyAsync(out + (size_t)e0 * npix, c->stage_out[slot].p, sizeof(float) * npix * n,
-                                        cudaMemcpyDeviceToHost, c->copy_stream));
+            CUDA_TRY(c, cudaMemcpyAsync(out + (size_t)e0 * npix, dst, sizeof(float) * npix * n, cudaMemcpyDeviceToHost, c->copy_stream));
             CUDA_TRY(c, cudaEventRecord(c->ev_copy[slot], c->copy_stream));
         }
         c->last_batch_e = n;

@@ -162,6 +162,131 @@ k_xpass_chi(const __grid_constant__ MorphPtrs mp, const float *__restrict__ coef
 }
 
 // ------------------------------------------------------------------------------------------
+// x pass, SPECTRAL_BASIS algorithm (DESIGN 7.2).  p is linear in the optical constants, so
+// the energy-independent REAL fields
+//   aligned material m:  phi, w = phi S, w dx dx, w dy dy, w dx dy, w dx dz, w dy dz   (7)
+//   isotropic material:  phi                                                           (1)
+// are transformed once per run.  Two real fields share one complex transform (field 2j in
+// the real part of pack j, field 2j+1 in the imaginary part); the Ewald kernel separates them
+// with F_a(q) = (Z(q) + conj Z(-q))/2, F_b(q) = (Z(q) - conj Z(-q))/(2i).
+// Materials are split into groups of at most 16 fields (8 packs); blockIdx.y = group.
+constexpr int BASIS_MAX_FIELDS = 16;
+constexpr int BASIS_MAX_PACKS = BASIS_MAX_FIELDS / 2;
+constexpr int BASIS_MAX_GROUPS = 16;
+enum BasisKind : int { BK_NONE = 0, BK_PHI, BK_W, BK_XX, BK_YY, BK_XY, BK_XZ, BK_YZ };
+
+struct BasisGroup {
+    int n_mat;
+    int mat[BASIS_MAX_FIELDS];
+    int n_fields;                 // 7 per aligned + 1 per isotropic material
+    int pack0;                    // first pack of this group in the spectrum buffer
+};
+struct BasisGroups {
+    int n_groups;
+    BasisGroup g[BASIS_MAX_GROUPS];
+};
+
+template <int LOGN> struct XBasisCfg {
+    static constexpr int N = 1 << LOGN;
+    static constexpr int TPR = XCfg<LOGN>::TPR, ROWS = XCfg<LOGN>::ROWS, THREADS = XCfg<LOGN>::THREADS;
+    static constexpr int CHUNK = 4;                                    // packs per fft_lines call
+    static constexpr int LS = RowLayout<N>::LS;
+    static constexpr size_t SMEM = sizeof(float) * 2 * (size_t)(ROWS * BASIS_MAX_PACKS) * LS + sizeof(float2) * N;
+};
+
+template <int LOGN>
+__global__ void __launch_bounds__(XBasisCfg<LOGN>::THREADS)
+k_xpass_basis(const __grid_constant__ MorphPtrs mp, const __grid_constant__ BasisGroups groups,
+              float2 *__restrict__ out, int rows_total, Window wx, int pitch, const float2 *__restrict__ tw_g)
+{
+    using Cfg = XBasisCfg<LOGN>;
+    constexpr int N = Cfg::N, ROWS = Cfg::ROWS, LS = Cfg::LS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float *re = reinterpret_cast<float *>(smem_raw);
+    float *im = re + ROWS * BASIS_MAX_PACKS * LS;
+    float2 *tw = reinterpret_cast<float2 *>(im + ROWS * BASIS_MAX_PACKS * LS);
+
+    const int tid = threadIdx.x;
+    const BasisGroup &G = groups.g[blockIdx.y];
+    const int row0 = blockIdx.x * ROWS;
+    const int nrows = min(ROWS, rows_total - row0);
+    const int npk = (G.n_fields + 1) >> 1;
+
+    for (int i = tid; i < N; i += Cfg::THREADS) tw[i] = tw_g[i];
+
+    const int rr = tid / Cfg::TPR, tx = tid % Cfg::TPR;
+    constexpr int NV = N >= 4 ? 4 : N;
+    int pos[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) pos[v] = RowLayout<N>::input_pos(4 * tx + v);
+    auto put = [&](int fi, int v, float val) {
+        float *arr = (fi & 1) ? im : re;
+        arr[((fi >> 1) * ROWS + rr) * LS + pos[v]] = val;
+    };
+    if (rr < nrows) {
+        const size_t base = (size_t)(row0 + rr) * N + 4 * tx;
+        int fi = 0;
+        for (int mi = 0; mi < G.n_mat; ++mi) {
+            const int m = G.mat[mi];
+            const bool aligned = mp.S[m] != nullptr;
+            const float4 p4 = __ldg(reinterpret_cast<const float4 *>(mp.phi[m] + base));
+            const float ph[4] = {p4.x, p4.y, p4.z, p4.w};
+            if (aligned) {
+                const float4 s4 = __ldg(reinterpret_cast<const float4 *>(mp.S[m] + base));
+                const float4 t4 = __ldg(reinterpret_cast<const float4 *>(mp.theta[m] + base));
+                const float4 q4 = __ldg(reinterpret_cast<const float4 *>(mp.psi[m] + base));
+                const float s[4] = {s4.x, s4.y, s4.z, s4.w}, th[4] = {t4.x, t4.y, t4.z, t4.w}, ps[4] = {q4.x, q4.y, q4.z, q4.w};
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    const float w = ph[v] * s[v];
+                    float st, ct, sp, cp;
+                    sincosf(th[v], &st, &ct);
+                    sincosf(ps[v], &sp, &cp);
+                    const float dx = cp * st, dy = sp * st, dz = ct;
+                    const float wx_ = w * dx, wy_ = w * dy;
+                    put(fi + 0, v, ph[v]); put(fi + 1, v, w);
+                    put(fi + 2, v, wx_ * dx); put(fi + 3, v, wy_ * dy);
+                    put(fi + 4, v, wx_ * dy); put(fi + 5, v, wx_ * dz); put(fi + 6, v, wy_ * dz);
+                }
+                fi += 7;
+            } else {
+#pragma unroll
+                for (int v = 0; v < NV; ++v) put(fi, v, ph[v]);
+                fi += 1;
+            }
+        }
+        if (fi & 1) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) put(fi, v, 0.f);
+        }
+    } else {
+        // unused rows of a ragged last CTA: keep them finite
+        for (int pk = 0; pk < npk; ++pk)
+#pragma unroll
+            for (int v = 0; v < NV; ++v) { re[(pk * ROWS + rr) * LS + pos[v]] = 0.f; im[(pk * ROWS + rr) * LS + pos[v]] = 0.f; }
+    }
+    __syncthreads();
+
+    for (int c0 = 0; c0 < npk; c0 += Cfg::CHUNK) {
+        RowAcc<N> racc{re + c0 * ROWS * LS, im + c0 * ROWS * LS};
+        fft_lines<LOGN, Cfg::CHUNK * ROWS, Cfg::THREADS>(racc, min(Cfg::CHUNK, npk - c0) * ROWS, tw, tid);
+    }
+
+    const size_t fstride = (size_t)rows_total * pitch;
+    for (int idx = tid; idx < npk * nrows * pitch; idx += Cfg::THREADS) {
+        const int lr = idx / pitch, sl = idx - lr * pitch;
+        const int pk = lr / nrows, r = lr - pk * nrows;
+        float2 val = make_float2(0.f, 0.f);
+        if (sl < wx.W) {
+            const int b = (wx.lo + sl) & (N - 1);
+            const int p = (pk * ROWS + r) * LS + RowLayout<N>::pos(b);
+            val = make_float2(re[p], im[p]);
+        }
+        out[(size_t)(G.pack0 + pk) * fstride + (size_t)(row0 + r) * pitch + sl] = val;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // Strided pass (z or y): a CTA loads a tile of N rows x TX contiguous columns, transforms the
 // TX columns, stores the rows whose bins lie in the window.  Batches: blockIdx.x = tile +
 // n_tiles * lo, blockIdx.y = hi, with separate in/out strides (in float2 units).
@@ -314,6 +439,70 @@ k_ewald_chi(const EwaldParams p)
 #pragma unroll
             for (int f = 0; f < NCHI; ++f)
                 c[f] = (inwin && sz < p.wz.W) ? __ldg(base + f * fstride + (size_t)sz * plane) : make_float2(0.f, 0.f);
+            const float2 u[3] = {c[0], c[1], c[2]}, v[3] = {c[1], c[3], c[4]};
+            float sxx, syy, sxy;
+            project_pair(g.r, u, v, sxx, syy, sxy);
+            const float w = g.wt[j] * k4;
+            axx = fmaf(w, sxx, axx); ayy = fmaf(w, syy, ayy); axy = fmaf(w, sxy, axy);
+        }
+    }
+    p.img[((size_t)e * p.Ny + iy) * p.Nx + ix] = make_float4(axx, ayy, axy, valid ? 1.f : 0.f);
+}
+
+// Ewald projection for SPECTRAL_BASIS: chi~(q) = sum_b coef[e][b] F_b(q) on the shell only.
+struct EwaldBasisParams {
+    EwaldParams g;              // geometry, windows, spec = packed spectra [pack][wz][wy][pitch], img
+    int n_pack;
+    const float2 *coef;         // [n_energy][2 n_pack], already multiplied by 1/2 (the unpacking factor)
+    const int *kind;            // [2 n_pack] BasisKind
+};
+
+__global__ void __launch_bounds__(256)
+k_ewald_basis(const EwaldBasisParams q)
+{
+    const EwaldParams &p = q.g;
+    const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int iy = blockIdx.y * 8 + (threadIdx.x >> 5);
+    const int e = blockIdx.z;
+    if (ix >= p.Nx || iy >= p.Ny) return;
+    const double k = p.k[p.e0 + e];
+    const PixelGeom g = pixel_geometry(ix, iy, p.Nx, p.Ny, p.Nz, p.mode, p.dqx, p.dqy, p.dqz, k);
+    float axx = 0.f, ayy = 0.f, axy = 0.f;
+    const bool valid = g.n_nodes > 0;
+    if (valid) {
+        const int mx = ix - p.Nx / 2, my = iy - p.Ny / 2;
+        const int sx = win_slot(p.wx, mx), sy = win_slot(p.wy, my);
+        const int tx = win_slot(p.wx, -mx), ty = win_slot(p.wy, -my);
+        const size_t plane = (size_t)p.wy.W * p.pitch;
+        const size_t fstride = plane * p.wz.W;
+        const bool inwin = sx < p.wx.W && sy < p.wy.W && tx < p.wx.W && ty < p.wy.W;
+        const double k2 = k * k;
+        const float k4 = (float)(k2 * k2);
+        const float2 *coef = q.coef + (size_t)(p.e0 + e) * 2 * q.n_pack;
+        for (int j = 0; j < g.n_nodes; ++j) {
+            const int sz = win_slot(p.wz, g.node[j]), tz = win_slot(p.wz, -g.node[j]);
+            const bool ok = inwin && sz < p.wz.W && tz < p.wz.W;
+            const float2 *pq = p.spec + (size_t)sz * plane + (size_t)sy * p.pitch + sx;
+            const float2 *pm = p.spec + (size_t)tz * plane + (size_t)ty * p.pitch + tx;
+            float2 c[NCHI];
+#pragma unroll
+            for (int f = 0; f < NCHI; ++f) c[f] = make_float2(0.f, 0.f);
+            for (int pk = 0; ok && pk < q.n_pack; ++pk) {
+                const float2 z1 = __ldg(pq + pk * fstride), z2 = __ldg(pm + pk * fstride);
+                // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
+                const float2 F[2] = {make_float2(z1.x + z2.x, z1.y - z2.y), make_float2(z1.y + z2.y, z2.x - z1.x)};
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int kd = __ldg(q.kind + 2 * pk + h);
+                    const float2 v = cmul(__ldg(coef + 2 * pk + h), F[h]);
+                    if (kd == BK_PHI || kd == BK_W) { c[0] = cadd(c[0], v); c[3] = cadd(c[3], v); }
+                    else if (kd == BK_XX) c[0] = cadd(c[0], v);
+                    else if (kd == BK_YY) c[3] = cadd(c[3], v);
+                    else if (kd == BK_XY) c[1] = cadd(c[1], v);
+                    else if (kd == BK_XZ) c[2] = cadd(c[2], v);
+                    else if (kd == BK_YZ) c[4] = cadd(c[4], v);
+                }
+            }
             const float2 u[3] = {c[0], c[1], c[2]}, v[3] = {c[1], c[3], c[4]};
             float sxx, syy, sxy;
             project_pair(g.r, u, v, sxx, syy, sxy);

@@ -8,7 +8,7 @@ from tests.parity import compare, oracle_run
 
 pytestmark = pytest.mark.gpu
 
-ALGS = [1]      # binding.ALG_PER_ENERGY; SPECTRAL_BASIS is added when built
+ALGS = [1, 2]      # binding.ALG_PER_ENERGY, binding.ALG_SPECTRAL_BASIS
 
 
 def _gpu(w, alg, images=False):
