@@ -14,6 +14,7 @@
 
 #include "../../include/cyrsoxs.h"
 #include "kernels.cuh"
+#include "kernels2.cuh"
 
 using namespace cyr;
 
@@ -32,7 +33,7 @@ struct DevBuf {
 } // namespace
 
 struct cyrsoxs_ctx {
-    int Nx = 0, Ny = 0, Nz = 0, n_mat = 0, device = 0;
+    int Nx = 0, Ny = 0, Nz = 0, n_mat = 0, device = 0, n_sm = 148;
     float voxel = 0.f;
     double dqx = 0, dqy = 0, dqz = 0;
     // morphology
@@ -43,7 +44,7 @@ struct cyrsoxs_ctx {
     int nE = 0;
     std::vector<double> energies, k;
     std::vector<float> coef;           // [nE][n_mat][6]: Cc, Ca, Cb (complex) / 4 pi
-    DevBuf d_coef, d_k;
+    DevBuf d_coef, d_k, d_reach2;
     bool have_optics = false;
     // angles
     int nA = 0;
@@ -203,15 +204,16 @@ cyrsoxs_status launch_xpass(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, flo
 
 template <int LOGN> cyrsoxs_status launch_colpass_t(cyrsoxs_ctx *c, cudaStream_t st, ColParams p, int n_lo, int n_hi, int pitch)
 {
-    using Cfg = ColCfg<LOGN>;
+    using Cfg = Col2Cfg<LOGN>;
     static bool attr_done[64] = {false};
     if (!attr_done[c->device & 63]) {
-        CUDA_TRY(c, cudaFuncSetAttribute(k_colpass<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        if (Cfg::SMEM > 48 * 1024)
+            CUDA_TRY(c, cudaFuncSetAttribute(k_col2<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
         attr_done[c->device & 63] = true;
     }
     p.n_tiles = pitch / Cfg::TX;
     dim3 grid((unsigned)(p.n_tiles * n_lo), (unsigned)n_hi);
-    k_colpass<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    k_col2<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
     CUDA_TRY(c, cudaGetLastError());
     return CYRSOXS_OK;
 }
@@ -255,6 +257,28 @@ void clear_prof(cyrsoxs_ctx *c)
     for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
     c->prof_events.clear();
     c->prof_stage.clear();
+}
+
+// Rotate back + average for energies [e0, e0 + eb) of the image buffer.  Energies per thread:
+// as many as still leave a few CTAs per SM.
+cyrsoxs_status launch_rotate(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, float *d_out, unsigned int *d_cnt)
+{
+    StageTimer t(c, st, CYRSOXS_STAGE_ROTATE);
+    RotateParams p{};
+    p.Nx = c->Nx; p.Ny = c->Ny; p.n_angles = c->nA; p.n_energy = eb;
+    p.cs = (const double2 *)c->d_cs.p; p.csf = (const float4 *)c->d_csf.p;
+    p.img = (const float4 *)c->img.p; p.out = d_out; p.counts = d_cnt;
+    p.reach2 = (const float *)c->d_reach2.p + e0;
+    p.rho = (double)c->Nx / (double)c->Ny;
+    const unsigned gx = (c->Nx + 31) / 32, gy = (c->Ny + 3) / 4;
+    const long long tiles = (long long)gx * gy;
+    const long long want = 8LL * c->n_sm;
+    if (eb >= 4 && tiles * ((eb + 3) / 4) >= want) k_rotate_avg<4><<<dim3(gx, gy, (eb + 3) / 4), 128, 0, st>>>(p);
+    else if (eb >= 2 && tiles * ((eb + 1) / 2) >= want) k_rotate_avg<2><<<dim3(gx, gy, (eb + 1) / 2), 128, 0, st>>>(p);
+    else k_rotate_avg<1><<<dim3(gx, gy, eb), 128, 0, st>>>(p);
+    CUDA_TRY(c, cudaGetLastError());
+    c->stats.stage_bytes[CYRSOXS_STAGE_ROTATE] += eb * (20.0 * c->Nx * c->Ny);
+    return CYRSOXS_OK;
 }
 
 // One energy batch of the PER_ENERGY algorithm: fields -> x -> z -> y -> Ewald -> rotate.
@@ -315,31 +339,22 @@ cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int
         const double nodes = (c->Nz > 1 && c->ewald == CYRSOXS_EWALD_TRILINEAR) ? 2.0 : 1.0;
         c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * 0.785 * nodes * NCHI * 8.0 + 16.0 * c->Nx * c->Ny);
     }
-    {
-        StageTimer t(c, st, CYRSOXS_STAGE_ROTATE);
-        RotateParams p{};
-        p.Nx = c->Nx; p.Ny = c->Ny; p.n_angles = c->nA;
-        p.cs = (const double2 *)c->d_cs.p; p.csf = (const float4 *)c->d_csf.p;
-        p.img = (const float4 *)c->img.p; p.out = d_out; p.counts = d_cnt;
-        k_rotate_avg<<<g2, 256, 0, st>>>(p);
-        CUDA_TRY(c, cudaGetLastError());
-        c->stats.stage_bytes[CYRSOXS_STAGE_ROTATE] += eb * (20.0 * c->Nx * c->Ny);
-    }
-    return CYRSOXS_OK;
+    return launch_rotate(c, st, e0, eb, d_out, d_cnt);
 }
 
-template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, const BasisGroups &g, float2 *out,
+template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, const BasisGroups &, float2 *out,
                                                    const Window &wx, int pitch)
 {
-    using Cfg = XBasisCfg<LOGN>;
+    using Cfg = XB2Cfg<LOGN>;
     static bool attr_done[64] = {false};
     if (!attr_done[c->device & 63]) {
-        CUDA_TRY(c, cudaFuncSetAttribute(k_xpass_basis<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        if (Cfg::SMEM > 48 * 1024)
+            CUDA_TRY(c, cudaFuncSetAttribute(k_xbasis2<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
         attr_done[c->device & 63] = true;
     }
     const int rows = c->Ny * c->Nz;
-    dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS, g.n_groups);
-    k_xpass_basis<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(c->mp, g, out, rows, wx, pitch, (const float2 *)c->twx.p);
+    dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS);
+    k_xbasis2<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(c->mp, out, rows, wx, pitch, (const float2 *)c->twx.p);
     CUDA_TRY(c, cudaGetLastError());
     return CYRSOXS_OK;
 }
@@ -354,37 +369,19 @@ cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, const BasisGroups 
     return fail(c, CYRSOXS_ERR_INVALID_ARG, "unsupported Nx");
 }
 
-// Groups of materials with at most BASIS_MAX_FIELDS real basis fields each (7 per aligned, 1 per
-// isotropic material), every group padded to whole packs.  Also the per-field kind/material
-// tables and the per-energy complex coefficient of each field (times 1/2 for the unpacking).
+// The basis fields in material order (7 per aligned, 1 per isotropic material), two per complex
+// pack, the last pack padded; the per-field kind/material tables and the per-energy complex
+// coefficient of each field (times 1/2 for the unpacking).
 cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c)
 {
-    BasisGroups &G = c->groups;
-    memset(&G, 0, sizeof G);
+    memset(&c->groups, 0, sizeof c->groups);
     c->basis_kind.clear(); c->basis_mat.clear();
-    int pack = 0;
-    BasisGroup cur{};
-    cur.pack0 = 0;
-    auto flush = [&]() {
-        if (cur.n_mat == 0) return true;
-        if (G.n_groups >= BASIS_MAX_GROUPS) return false;
-        if (cur.n_fields & 1) { c->basis_kind.push_back(BK_NONE); c->basis_mat.push_back(0); }
-        pack += (cur.n_fields + 1) / 2;
-        G.g[G.n_groups++] = cur;
-        cur = BasisGroup{};
-        cur.pack0 = pack;
-        return true;
-    };
     for (int m = 0; m < c->n_mat; ++m) {
-        const bool aligned = c->mp.S[m] != nullptr;
-        const int nf = aligned ? 7 : 1;
-        if (cur.n_fields + nf > BASIS_MAX_FIELDS && !flush()) return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "too many basis groups");
-        cur.mat[cur.n_mat++] = m;
-        cur.n_fields += nf;
-        if (aligned) for (int kd = BK_PHI; kd <= BK_YZ; ++kd) { c->basis_kind.push_back(kd); c->basis_mat.push_back(m); }
+        if (c->mp.S[m] != nullptr) for (int kd = BK_PHI; kd <= BK_YZ; ++kd) { c->basis_kind.push_back(kd); c->basis_mat.push_back(m); }
         else { c->basis_kind.push_back(BK_PHI); c->basis_mat.push_back(m); }
     }
-    if (!flush()) return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "too many basis groups");
+    if (c->basis_kind.size() & 1) { c->basis_kind.push_back(BK_NONE); c->basis_mat.push_back(0); }
+    const int pack = (int)c->basis_kind.size() / 2;
     c->n_pack = pack;
     const int nb = 2 * pack;
     std::vector<float2> coef((size_t)c->nE * nb);
@@ -472,17 +469,7 @@ cyrsoxs_status run_batch_spectral(cyrsoxs_ctx *c, cudaStream_t st, int e0, int e
         const double nodes = (c->Nz > 1 && c->ewald == CYRSOXS_EWALD_TRILINEAR) ? 2.0 : 1.0;
         c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * 0.785 * nodes * 2.0 * c->n_pack * 8.0 + 16.0 * c->Nx * c->Ny);
     }
-    {
-        StageTimer t(c, st, CYRSOXS_STAGE_ROTATE);
-        RotateParams p{};
-        p.Nx = c->Nx; p.Ny = c->Ny; p.n_angles = c->nA;
-        p.cs = (const double2 *)c->d_cs.p; p.csf = (const float4 *)c->d_csf.p;
-        p.img = (const float4 *)c->img.p; p.out = d_out; p.counts = d_cnt;
-        k_rotate_avg<<<g2, 256, 0, st>>>(p);
-        CUDA_TRY(c, cudaGetLastError());
-        c->stats.stage_bytes[CYRSOXS_STAGE_ROTATE] += eb * (20.0 * c->Nx * c->Ny);
-    }
-    return CYRSOXS_OK;
+    return launch_rotate(c, st, e0, eb, d_out, d_cnt);
 }
 
 } // namespace
@@ -512,6 +499,7 @@ cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm,
     c->dqy = (2.0 * kPi) / ((double)Ny * (double)voxel_nm);
     c->dqz = (2.0 * kPi) / ((double)Nz * (double)voxel_nm);
     c->mp.n_mat = n_mat;
+    if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); c->n_sm = 148; }
     cyrsoxs_status st;
     if ((st = make_twiddles(c, c->twx, Nx)) != CYRSOXS_OK || (st = make_twiddles(c, c->twy, Ny)) != CYRSOXS_OK
         || (st = make_twiddles(c, c->twz, Nz)) != CYRSOXS_OK) {
@@ -527,7 +515,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
     if (!c) return;
     clear_prof(c);
     for (void *p : c->owned_morph) cudaFree(p);
-    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_cs, &c->d_csf, &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
+    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
                       &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind})
         release(*b);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
@@ -673,6 +661,17 @@ cyrsoxs_status cyrsoxs_set_optical_constants(cyrsoxs_ctx *c, int n_energy, const
     if ((st = ensure(c, c->d_k, sizeof(double) * n_energy)) != CYRSOXS_OK) return st;
     CUDA_TRY(c, cudaMemcpy(c->d_coef.p, c->coef.data(), sizeof(float) * c->coef.size(), cudaMemcpyHostToDevice));
     CUDA_TRY(c, cudaMemcpy(c->d_k.p, c->k.data(), sizeof(double) * n_energy, cudaMemcpyHostToDevice));
+    {
+        // reach of the valid disk in x pixels, see k_rotate_avg
+        std::vector<float> reach2(n_energy);
+        const double rho = (double)c->Nx / (double)c->Ny;
+        for (int e = 0; e < n_energy; ++e) {
+            const double r = c->k[e] / c->dqx + sqrt(1.0 + rho * rho) + 1.0;
+            reach2[e] = (float)(r * r * 1.0001);
+        }
+        if ((st = ensure(c, c->d_reach2, sizeof(float) * n_energy)) != CYRSOXS_OK) return st;
+        CUDA_TRY(c, cudaMemcpy(c->d_reach2.p, reach2.data(), sizeof(float) * n_energy, cudaMemcpyHostToDevice));
+    }
     c->have_optics = true;
     c->plan_dirty = true;
     return CYRSOXS_OK;

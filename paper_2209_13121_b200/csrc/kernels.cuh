@@ -514,58 +514,90 @@ k_ewald_basis(const EwaldBasisParams q)
 }
 
 // ------------------------------------------------------------------------------------------
-// Rotate back and average (DESIGN 3-A9/A10).  One thread per output pixel and energy; loops
-// over the angles.  cs[a] = (C, S) in double; csf[a] = (C^2, S^2, 2 C S) in float.
+// Rotate back and average (DESIGN 3-A9/A10).  One thread per output pixel and EPT energies:
+// the bilinear cell of an (output pixel, angle) pair is pure geometry (fp64, every operation
+// rounded on its own) and does not depend on the energy, so it is computed once and reused for
+// the EPT images the thread accumulates.  cs[a] = (C, S) in double; csf[a] = (C^2, S^2, 2 C S).
 struct RotateParams {
-    int Nx, Ny, n_angles;
+    int Nx, Ny, n_angles, n_energy;
     const double2 *cs;
     const float4 *csf;
     const float4 *img;          // [e][Ny][Nx]
     float *out;                 // [e][Ny][Nx]
     unsigned int *counts;       // optional
+    const float *reach2;        // [e] squared reach (in pixels of x) of the valid disk, see below
+    double rho;                 // Nx / Ny
 };
 
-__global__ void __launch_bounds__(256)
+// reach2[e] = (k_e/dq_x + 3)^2: an output pixel whose distance from q = 0 (measured in x
+// pixels, y pixels scaled by rho) exceeds the reach has every bilinear neighbour outside the
+// Ewald disk s^2 >= 0 at every angle (rotation keeps the distance, a cell adds < 2 pixels), so
+// its count is 0 and nothing needs to be read.  The margin of 3 keeps the decision away from
+// rounding: only pixels that are invalid with certainty are skipped.
+template <int EPT>
+__global__ void __launch_bounds__(128)
 k_rotate_avg(const RotateParams p)
 {
     const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
-    const int iy = blockIdx.y * 8 + (threadIdx.x >> 5);
-    const int e = blockIdx.z;
+    const int iy = blockIdx.y * 4 + (threadIdx.x >> 5);
+    const int e0 = blockIdx.z * EPT;
     if (ix >= p.Nx || iy >= p.Ny) return;
-    const float4 *img = p.img + (size_t)e * p.Ny * p.Nx;
-    const double rho = (double)p.Nx / (double)p.Ny;
+    const size_t plane = (size_t)p.Ny * p.Nx;
+    const float4 *img = p.img + (size_t)e0 * plane;
+    const int ne = min(EPT, p.n_energy - e0);
+    const double rho = p.rho;
     const double u = (double)(ix - p.Nx / 2), v = (double)(iy - p.Ny / 2);
     const double vr = v * rho, ur = u / rho;                 // exact: rho is a power of two
     const double cx = (double)(p.Nx / 2), cy = (double)(p.Ny / 2);
-    float sum = 0.f;
-    unsigned int cnt = 0;
-    for (int a = 0; a < p.n_angles; ++a) {
+    const float r2 = (float)(u * u + vr * vr);
+    float sum[EPT];
+    unsigned int cnt[EPT];
+    bool live[EPT];
+    bool any = false;
+#pragma unroll
+    for (int j = 0; j < EPT; ++j) {
+        sum[j] = 0.f; cnt[j] = 0;
+        live[j] = j < ne && r2 <= __ldg(p.reach2 + e0 + j);
+        any |= live[j];
+    }
+    for (int a = 0; any && a < p.n_angles; ++a) {
         const double2 cs = p.cs[a];
         const double fx = __dadd_rn(__dsub_rn(__dmul_rn(cs.x, u), __dmul_rn(cs.y, vr)), cx);
         const double fy = __dadd_rn(__dadd_rn(__dmul_rn(cs.y, ur), __dmul_rn(cs.x, v)), cy);
         const double x0 = floor(fx), y0 = floor(fy);
         const double al = fx - x0, be = fy - y0;
-        const int nx = al > 0.0 ? 2 : 1, ny = be > 0.0 ? 2 : 1;
-        if (x0 < 0.0 || y0 < 0.0 || x0 + (double)(nx - 1) > (double)(p.Nx - 1) || y0 + (double)(ny - 1) > (double)(p.Ny - 1))
+        const int dx = al > 0.0 ? 1 : 0, dy = be > 0.0 ? 1 : 0;    // a neighbour is needed iff its weight > 0
+        if (x0 < 0.0 || y0 < 0.0 || x0 + (double)dx > (double)(p.Nx - 1) || y0 + (double)dy > (double)(p.Ny - 1))
             continue;
         const int X0 = (int)x0, Y0 = (int)y0;
         const float4 w = p.csf[a];
         const float fa = (float)al, fb = (float)be;
-        float acc = 0.f;
-        bool ok = true;
-        for (int jy = 0; jy < ny; ++jy)
-            for (int jx = 0; jx < nx; ++jx) {
-                const float4 t = __ldg(img + (size_t)(Y0 + jy) * p.Nx + (X0 + jx));
-                ok = ok && (t.w != 0.f);
-                const float I = w.x * t.x + w.y * t.y + w.z * t.z;
-                const float wt = (jx ? fa : 1.f - fa) * (jy ? fb : 1.f - fb);
-                acc = fmaf(wt, I, acc);
+        const float w00 = (1.f - fa) * (1.f - fb), w10 = fa * (1.f - fb), w01 = (1.f - fa) * fb, w11 = fa * fb;
+        // un-needed neighbours alias a needed one (weight 0, same validity)
+        const float4 *p00 = img + (size_t)Y0 * p.Nx + X0;
+        const float4 *p10 = p00 + dx, *p01 = p00 + (size_t)dy * p.Nx, *p11 = p01 + dx;
+#pragma unroll
+        for (int j = 0; j < EPT; ++j) {
+            if (live[j]) {
+                const float4 t00 = __ldg(p00 + j * plane), t10 = __ldg(p10 + j * plane);
+                const float4 t01 = __ldg(p01 + j * plane), t11 = __ldg(p11 + j * plane);
+                const bool ok = (t00.w != 0.f) & (t10.w != 0.f) & (t01.w != 0.f) & (t11.w != 0.f);
+                float acc = w00 * (w.x * t00.x + w.y * t00.y + w.z * t00.z);
+                acc = fmaf(w10, w.x * t10.x + w.y * t10.y + w.z * t10.z, acc);
+                acc = fmaf(w01, w.x * t01.x + w.y * t01.y + w.z * t01.z, acc);
+                acc = fmaf(w11, w.x * t11.x + w.y * t11.y + w.z * t11.z, acc);
+                if (ok) { sum[j] += acc; ++cnt[j]; }
             }
-        if (ok) { sum += acc; ++cnt; }
+        }
     }
-    const size_t o = ((size_t)e * p.Ny + iy) * p.Nx + ix;
-    p.out[o] = cnt ? sum / (float)cnt : 0.f;
-    if (p.counts) p.counts[o] = cnt;
+#pragma unroll
+    for (int j = 0; j < EPT; ++j) {
+        if (j < ne) {
+            const size_t o = ((size_t)(e0 + j) * p.Ny + iy) * p.Nx + ix;
+            p.out[o] = cnt[j] ? sum[j] / (float)cnt[j] : 0.f;
+            if (p.counts) p.counts[o] = cnt[j];
+        }
+    }
 }
 
 } // namespace cyr

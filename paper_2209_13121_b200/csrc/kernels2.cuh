@@ -1,0 +1,223 @@
+// kernels2.cuh -- second-generation FFT passes built on fft_reg.cuh (register-first /
+// register-last): the strided z / y pass (k_col2) and the SPECTRAL_BASIS x pass (k_xbasis2).
+#pragma once
+#include "fft_reg.cuh"
+#include "kernels.cuh"
+
+namespace cyr {
+
+// ------------------------------------------------------------------------------------------
+// Strided pass (z or y).  A CTA transforms a tile of TX adjacent columns (contiguous along x)
+// by N rows of one (lo, hi) batch item.  Thread (li, c): c = tid % TX is the column, li the
+// butterfly index.  Loads go straight from global memory into the stage-0 registers (lanes
+// run along x: TX * 8 contiguous bytes per row), the last stage stores straight to global,
+// pruned to the window.  Same parameters and batch mapping as k_colpass (ColParams).
+template <int LOGN> struct Col2Cfg {
+    static constexpr int N = 1 << LOGN;
+    static constexpr int TX = N <= 256 ? 16 : (N <= 1024 ? 8 : 4);
+    using F = RegFft<LOGN, ColMap<TX>>;
+    static constexpr int T = F::T;
+    static constexpr int THREADS = T * TX;
+    static constexpr size_t SMEM = F::NST > 1 ? sizeof(float2) * (size_t)N * TX : 0;
+};
+
+template <int LOGN>
+__global__ void __launch_bounds__(Col2Cfg<LOGN>::THREADS)
+k_col2(const ColParams p)
+{
+    using Cfg = Col2Cfg<LOGN>;
+    using F = typename Cfg::F;
+    constexpr int N = Cfg::N, TX = Cfg::TX, T = Cfg::T, R0 = F::R0, NST = F::NST;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw);
+    const int tid = threadIdx.x;
+    const int c = tid % TX, li = tid / TX;
+    const int tile = blockIdx.x % p.n_tiles, lo = blockIdx.x / p.n_tiles, hi = blockIdx.y;
+
+    const float2 *src = p.in + (size_t)hi * p.in_hi + (size_t)lo * p.in_lo + (size_t)tile * TX + c;
+    float2 v[R0];
+#pragma unroll
+    for (int s = 0; s < R0; ++s) v[s] = __ldcs(src + (size_t)(li + s * T) * p.in_row);
+    F::stage0(v);
+    float2 *L = sm + c;
+    if constexpr (NST > 1) {
+        F::stage0_store(L, li, v);
+        float2 w[R0];
+        if constexpr (NST > 2) {
+            __syncthreads();
+            F::template load_tw<1>(p.tw, li, w);
+            F::template stage_load<1>(L, li, w, v);
+            __syncthreads();
+            F::template stage_store<1>(L, li, v);
+        }
+        if constexpr (NST > 3) {
+            __syncthreads();
+            F::template load_tw<2>(p.tw, li, w);
+            F::template stage_load<2>(L, li, w, v);
+            __syncthreads();
+            F::template stage_store<2>(L, li, v);
+        }
+        __syncthreads();
+        F::template load_tw<NST - 1>(p.tw, li, w);
+        F::template stage_load<NST - 1>(L, li, w, v);
+    }
+    float2 *dst = p.out + (size_t)hi * p.out_hi + (size_t)lo * p.out_lo + (size_t)tile * TX + c;
+#pragma unroll
+    for (int m = 0; m < R0; ++m) {
+        const int k = li + T * m;
+        const int sl = (k - p.win.lo) & (N - 1);
+        if (sl < p.win.W) dst[(size_t)sl * p.out_row] = v[F::out_reg(m)];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// x pass of SPECTRAL_BASIS (DESIGN 7.2).  The energy-independent real fields, in material order
+//   aligned material:   phi, w = phi S, w dx dx, w dy dy, w dx dy, w dx dz, w dy dz      (7)
+//   isotropic material: phi                                                              (1)
+// form one global sequence; consecutive fields 2j, 2j+1 are the real and imaginary part of
+// complex pack j (the last pack is padded with zeros).  T = N / R0 threads share a row; a thread
+// owns the voxels x = li + s T (s < R0), generates their fields in registers, runs the stage-0
+// butterfly there, and the remaining stages through a 4-pack shared-memory buffer per row; the
+// last stage stores the window [lo, lo + W) of bins straight to out[pack][row][slot].
+constexpr int XB2_PB = 4;       // packs buffered per row between flushes
+
+template <int LOGN> struct XB2Cfg {
+    static constexpr int N = 1 << LOGN;
+    using F = RegFft<LOGN, RowMap>;
+    static constexpr int T = F::T, R0 = F::R0;
+    static constexpr int ROWS = T >= 256 ? 1 : 256 / T;
+    static constexpr int THREADS = ROWS * T;
+    static constexpr size_t SMEM = F::NST > 1 ? sizeof(float2) * (size_t)ROWS * XB2_PB * N : 0;
+};
+
+template <int LOGN>
+__global__ void __launch_bounds__(XB2Cfg<LOGN>::THREADS, 2)
+k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, Window wx, int pitch,
+          const float2 *__restrict__ tw)
+{
+    using Cfg = XB2Cfg<LOGN>;
+    using F = typename Cfg::F;
+    constexpr int N = Cfg::N, T = Cfg::T, R0 = Cfg::R0, NST = F::NST, THREADS = Cfg::THREADS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x;
+    const int g = tid / T, li = tid % T;
+    const int row = blockIdx.x * Cfg::ROWS + g;
+    const bool row_ok = row < rows_total;
+    const int rowc = row_ok ? row : rows_total - 1;
+    float2 *Lrow = reinterpret_cast<float2 *>(smem_raw) + (size_t)g * (XB2_PB * N);
+    const size_t vox0 = (size_t)rowc * N + li;
+    const size_t fstride = (size_t)rows_total * pitch;
+    float2 *orow = out + (size_t)rowc * pitch;
+
+    float carry[R0];
+    bool has_carry = false;
+    int nbuf = 0, pack_out = 0;
+
+    auto store_global = [&](int pack, const float2 (&v)[R0]) {
+        float2 *o = orow + (size_t)pack * fstride;
+#pragma unroll
+        for (int m = 0; m < R0; ++m) {
+            const int k = li + T * m;
+            const int sl = (k - wx.lo) & (N - 1);
+            if (sl < pitch && row_ok) o[sl] = sl < wx.W ? v[F::out_reg(m)] : make_float2(0.f, 0.f);
+        }
+        if (N < 32) {
+            for (int sl = N + li; sl < pitch; sl += T)
+                if (row_ok) o[sl] = make_float2(0.f, 0.f);
+        }
+    };
+    auto emit = [&](const float (&a)[R0], const float (&b)[R0]) {
+        float2 v[R0];
+#pragma unroll
+        for (int s = 0; s < R0; ++s) v[s] = make_float2(a[s], b[s]);
+        F::stage0(v);
+        if constexpr (NST > 1) { F::stage0_store(Lrow + nbuf * N, li, v); ++nbuf; }
+        else { store_global(pack_out, v); ++pack_out; }
+    };
+    auto flush = [&]() {
+        if constexpr (NST > 1) {
+            float2 w[R0], v[R0];
+            if constexpr (NST > 2) {
+                group_sync<T, THREADS>(g);
+                F::template load_tw<1>(tw, li, w);
+                for (int pk = 0; pk < nbuf; ++pk) {
+                    F::template stage_load<1>(Lrow + pk * N, li, w, v);
+                    group_sync<T, THREADS>(g);
+                    F::template stage_store<1>(Lrow + pk * N, li, v);
+                }
+            }
+            if constexpr (NST > 3) {
+                group_sync<T, THREADS>(g);
+                F::template load_tw<2>(tw, li, w);
+                for (int pk = 0; pk < nbuf; ++pk) {
+                    F::template stage_load<2>(Lrow + pk * N, li, w, v);
+                    group_sync<T, THREADS>(g);
+                    F::template stage_store<2>(Lrow + pk * N, li, v);
+                }
+            }
+            group_sync<T, THREADS>(g);
+            F::template load_tw<NST - 1>(tw, li, w);
+            for (int pk = 0; pk < nbuf; ++pk) {
+                F::template stage_load<NST - 1>(Lrow + pk * N, li, w, v);
+                store_global(pack_out + pk, v);
+            }
+            group_sync<T, THREADS>(g);          // the buffer is reused by the next stage-0 stores
+            pack_out += nbuf;
+            nbuf = 0;
+        }
+    };
+
+    for (int m = 0; m < mp.n_mat; ++m) {
+        const bool aligned = mp.S[m] != nullptr;
+        if (nbuf + (aligned ? 4 : 1) > XB2_PB) flush();
+        float ph[R0];
+#pragma unroll
+        for (int s = 0; s < R0; ++s) ph[s] = __ldg(mp.phi[m] + vox0 + (size_t)s * T);
+        if (aligned) {
+            float S_[R0], th[R0], ps[R0];
+#pragma unroll
+            for (int s = 0; s < R0; ++s) {
+                S_[s] = __ldg(mp.S[m] + vox0 + (size_t)s * T);
+                th[s] = __ldg(mp.theta[m] + vox0 + (size_t)s * T);
+                ps[s] = __ldg(mp.psi[m] + vox0 + (size_t)s * T);
+            }
+            float fw[R0], fxx[R0], fyy[R0], fxy[R0], fxz[R0], fyz[R0];
+#pragma unroll
+            for (int s = 0; s < R0; ++s) {
+                const float w = ph[s] * S_[s];
+                float st, ct, sp, cp;
+                sincosf(th[s], &st, &ct);
+                sincosf(ps[s], &sp, &cp);
+                const float dx = cp * st, dy = sp * st, dz = ct;
+                const float wdx = w * dx, wdy = w * dy;
+                fw[s] = w; fxx[s] = wdx * dx; fyy[s] = wdy * dy; fxy[s] = wdx * dy; fxz[s] = wdx * dz; fyz[s] = wdy * dz;
+            }
+            if (has_carry) {
+                emit(carry, ph); emit(fw, fxx); emit(fyy, fxy); emit(fxz, fyz);
+                has_carry = false;
+            } else {
+                emit(ph, fw); emit(fxx, fyy); emit(fxy, fxz);
+#pragma unroll
+                for (int s = 0; s < R0; ++s) carry[s] = fyz[s];
+                has_carry = true;
+            }
+        } else {
+            if (has_carry) { emit(carry, ph); has_carry = false; }
+            else {
+#pragma unroll
+                for (int s = 0; s < R0; ++s) carry[s] = ph[s];
+                has_carry = true;
+            }
+        }
+    }
+    if (has_carry) {
+        if (nbuf + 1 > XB2_PB) flush();
+        float zero[R0];
+#pragma unroll
+        for (int s = 0; s < R0; ++s) zero[s] = 0.f;
+        emit(carry, zero);
+    }
+    flush();
+}
+
+} // namespace cyr
