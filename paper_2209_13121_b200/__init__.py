@@ -5,4 +5,4 @@ layer over the C-ABI library `libcyrsoxs.so` declared in include/cyrsoxs.h.  Imp
 the package does not load the library; `binding.load()` does and fails loudly if the
 CUDA build is missing (there is no CPU fallback).
 """
-__all__ = ["workloads", "binding", "build"]
+__all__ = ["workloads", "binding", "build", "sharding"]

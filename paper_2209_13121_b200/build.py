@@ -15,7 +15,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libcyrsoxs.so"
 SOURCES = [CSRC / "cyrsoxs_api.cu"]
-HEADERS = [CSRC / "kernels.cuh", CSRC / "fft_core.cuh", PKG.parent / "include" / "cyrsoxs.h"]
+HEADERS = sorted(CSRC.glob("*.cuh")) + [PKG.parent / "include" / "cyrsoxs.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
