@@ -67,24 +67,53 @@ def make_workload(name: str, rank: int, world: int):
 
 
 class ClockSampler(threading.Thread):
-    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    """Samples SM clock, power and throttle reasons while the timed region runs.  Uses NVML in
+    process (pynvml); spawning nvidia-smi every 100 ms stalls kernel launches of a 0.15 ms step
+    for milliseconds, so it is only the fallback."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
         self.index, self.rows, self.stop_flag = index, [], False
+        self.nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and all(x.strip().isdigit() for x in vis.split(",")) else index
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.nvml = pynvml
+        except Exception:
+            self.nvml = None
 
-    def run(self):
-        while not self.stop_flag:
-            try:
+    def _sample_nvml(self):
+        n, h = self.nvml, self.handle
+        sm = n.nvmlDeviceGetClockInfo(h, n.NVML_CLOCK_SM)
+        mx = n.nvmlDeviceGetMaxClockInfo(h, n.NVML_CLOCK_SM)
+        pw = n.nvmlDeviceGetPowerUsage(h) / 1000.0
+        r = n.nvmlDeviceGetCurrentClocksEventReasons(h) if hasattr(n, "nvmlDeviceGetCurrentClocksEventReasons") \
+            else n.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+        bits = [getattr(n, "nvmlClocksThrottleReasonHwSlowdown", 0x8), getattr(n, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                getattr(n, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20), getattr(n, "nvmlClocksThrottleReasonSwPowerCap", 0x4)]
+        return [str(sm), str(mx), str(pw)] + ["Active" if r & b else "Not Active" for b in bits]
+
+    def sample_once(self):
+        try:
+            if self.nvml is not None:
+                self.rows.append(self._sample_nvml())
+            else:
                 o = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
                                    capture_output=True, text=True, timeout=5).stdout.strip()
                 if o:
                     self.rows.append([x.strip() for x in o.split(",")])
-            except Exception:
-                pass
-            time.sleep(0.1)
+        except Exception:
+            pass
+
+    def run(self):
+        while not self.stop_flag:
+            self.sample_once()
+            time.sleep(0.005 if self.nvml is not None else 0.1)
 
     def summary(self):
         if not self.rows:
@@ -93,7 +122,8 @@ class ClockSampler(threading.Thread):
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = [n for j, n in enumerate(names) if any(r[3 + j].lower().startswith("active") for r in self.rows)]
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
-                "samples": len(sm), "power_w_max": max(float(r[2]) for r in self.rows)}
+                "samples": len(sm), "power_w_max": max(float(r[2]) for r in self.rows),
+                "source": "nvml" if self.nvml is not None else "nvidia-smi"}
 
 
 def oracle_sample(w, budget_s: float = 20.0):
@@ -177,6 +207,8 @@ def run_ours(args, rank, world, local_rank):
     sampler = ClockSampler(local_rank)
     sampler.start()
     evs = [one_step() for _ in range(args.steps)]
+    if sampler.nvml is not None:
+        sampler.sample_once()                           # at least one sample while the queue is still draining
     barrier()
     sampler.stop_flag = True
     sampler.join(timeout=3)

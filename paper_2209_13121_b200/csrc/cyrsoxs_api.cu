@@ -6,10 +6,12 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include <algorithm>
 #include <complex>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/cyrsoxs.h"
@@ -49,7 +51,12 @@ struct cyrsoxs_ctx {
     // angles
     int nA = 0;
     std::vector<double2> cs;
-    DevBuf d_cs, d_csf;
+    DevBuf d_cs, d_csf, d_tiles[4];            // rotate tile tables for EG = 1, 2, 4, 8
+    int n_tiles[4] = {0, 0, 0, 0};
+    int eg = 1;                                 // energies interleaved per image group in this run
+    unsigned long long plan_key = 0;            // what the cached energy batch was planned for
+    size_t plan_fixed = 0, plan_per_e = 0;
+    int plan_eb = 0;
     bool have_angles = false;
     // options
     int ewald = CYRSOXS_EWALD_TRILINEAR;
@@ -156,12 +163,44 @@ Window make_window(int N, int K, bool symmetric)
 
 int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
-struct Plan {
-    Window wx, wy, wz;
-    int pitch;
-    int eb;                    // energies per batch
-    size_t a1, a2, a3, img;    // float2 / float2 / float2 / float4 element counts per batch
-};
+// Output tiles of the rotate kernel for image layout EG = 1 << lg, nearest to q = 0 first
+// (see k_rotate_avg); built on first use.
+cyrsoxs_status make_rotate_tiles(cyrsoxs_ctx *c, int lg)
+{
+    if (c->n_tiles[lg]) return CYRSOXS_OK;
+    const int TW = lg == 0 ? RotMap<1>::TW : lg == 1 ? RotMap<2>::TW : lg == 2 ? RotMap<4>::TW : RotMap<8>::TW;
+    const int TH = lg == 0 ? RotMap<1>::TH : lg == 1 ? RotMap<2>::TH : lg == 2 ? RotMap<4>::TH : RotMap<8>::TH;
+    const int ntx = (c->Nx + TW - 1) / TW, nty = (c->Ny + TH - 1) / TH;
+    const double rho = (double)c->Nx / (double)c->Ny;
+    std::vector<std::pair<double, uint32_t>> t;
+    t.reserve((size_t)ntx * nty);
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < ntx; ++tx) {
+            const double ux = tx * TW + 0.5 * TW - c->Nx / 2, uy = (ty * TH + 0.5 * TH - c->Ny / 2) * rho;
+            t.emplace_back(ux * ux + uy * uy, ((uint32_t)ty << 16) | (uint32_t)tx);
+        }
+    std::sort(t.begin(), t.end());
+    std::vector<uint32_t> h(t.size());
+    for (size_t i = 0; i < t.size(); ++i) h[i] = t[i].second;
+    cyrsoxs_status st = ensure(c, c->d_tiles[lg], sizeof(uint32_t) * h.size());
+    if (st != CYRSOXS_OK) return st;
+    CUDA_TRY(c, cudaMemcpy(c->d_tiles[lg].p, h.data(), sizeof(uint32_t) * h.size(), cudaMemcpyHostToDevice));
+    c->n_tiles[lg] = (int)h.size();
+    return CYRSOXS_OK;
+}
+
+// Energies interleaved per image group for a batch of eb energies: the largest of 8, 4, 2
+// whose padding (lanes of the last group without an energy) stays below a third, else 1.
+int choose_eg(int eb)
+{
+    static const int force = getenv("CYRSOXS_EG") ? atoi(getenv("CYRSOXS_EG")) : 0;      // tuning aid
+    if (force == 1 || force == 2 || force == 4 || force == 8) return force;
+    for (int eg = 8; eg >= 2; eg >>= 1) {
+        const int padded = (eb + eg - 1) / eg * eg;
+        if (3 * (padded - eb) <= padded) return eg;
+    }
+    return 1;
+}
 
 // Windows from the largest wavenumber in [e0, e1): valid pixels have |q_x|, |q_y| <= k and
 // k_z nodes in [-(k/dq_z) - 1, 0] (Eq. 8).  One extra bin of slack on every side.
@@ -259,8 +298,37 @@ void clear_prof(cyrsoxs_ctx *c)
     c->prof_stage.clear();
 }
 
-// Rotate back + average for energies [e0, e0 + eb) of the image buffer.  Energies per thread:
-// as many as still leave a few CTAs per SM.
+template <int EG> dim3 ewald_grid(const cyrsoxs_ctx *c, int eb)
+{
+    using M = EwaldMap<EG>;
+    return dim3((c->Nx + M::PW - 1) / M::PW, (c->Ny + M::PH - 1) / M::PH, (eb + EG - 1) / EG);
+}
+
+template <int EG>
+cyrsoxs_status launch_rotate_t(cyrsoxs_ctx *c, cudaStream_t st, RotateParams p, int eb, int lg)
+{
+    cyrsoxs_status s = make_rotate_tiles(c, lg);
+    if (s != CYRSOXS_OK) return s;
+    p.tiles = (const uint32_t *)c->d_tiles[lg].p;
+    const long long tiles = c->n_tiles[lg];
+    const int ng = (eb + EG - 1) / EG;
+    // groups per CTA: all of them (up to ROT_GMAX), so the cells of an angle are computed once per pixel
+    static const int force_ua = getenv("CYRSOXS_ROT_UA") ? atoi(getenv("CYRSOXS_ROT_UA")) : 0;      // tuning aid
+    const int gpc = std::min(ng, ROT_GMAX);
+    p.gpc = gpc;
+    const dim3 grid((unsigned)tiles, (ng + gpc - 1) / gpc);
+    const size_t smem = (size_t)gpc * 256 * 8;
+    // angles in flight: 1 when the grid fills the machine several times over (occupancy hides the
+    // load latency; measured best on cfg4), 4 when it does not (cfg1, cfg2)
+    const int ua = force_ua ? force_ua : ((long long)grid.x * grid.y >= 16LL * c->n_sm ? 1 : 4);
+    if (ua == 4) k_rotate_avg<EG, 4, 2><<<grid, 256, smem, st>>>(p);
+    else if (ua == 2) k_rotate_avg<EG, 2, 3><<<grid, 256, smem, st>>>(p);
+    else k_rotate_avg<EG, 1, 4><<<grid, 256, smem, st>>>(p);
+    CUDA_TRY(c, cudaGetLastError());
+    return CYRSOXS_OK;
+}
+
+// Rotate back + average for energies [e0, e0 + eb) of the image buffer.
 cyrsoxs_status launch_rotate(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, float *d_out, unsigned int *d_cnt)
 {
     StageTimer t(c, st, CYRSOXS_STAGE_ROTATE);
@@ -270,13 +338,14 @@ cyrsoxs_status launch_rotate(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, fl
     p.img = (const float4 *)c->img.p; p.out = d_out; p.counts = d_cnt;
     p.reach2 = (const float *)c->d_reach2.p + e0;
     p.rho = (double)c->Nx / (double)c->Ny;
-    const unsigned gx = (c->Nx + 31) / 32, gy = (c->Ny + 3) / 4;
-    const long long tiles = (long long)gx * gy;
-    const long long want = 8LL * c->n_sm;
-    if (eb >= 4 && tiles * ((eb + 3) / 4) >= want) k_rotate_avg<4><<<dim3(gx, gy, (eb + 3) / 4), 128, 0, st>>>(p);
-    else if (eb >= 2 && tiles * ((eb + 1) / 2) >= want) k_rotate_avg<2><<<dim3(gx, gy, (eb + 1) / 2), 128, 0, st>>>(p);
-    else k_rotate_avg<1><<<dim3(gx, gy, eb), 128, 0, st>>>(p);
-    CUDA_TRY(c, cudaGetLastError());
+    cyrsoxs_status s;
+    switch (c->eg) {
+    case 8: s = launch_rotate_t<8>(c, st, p, eb, 3); break;
+    case 4: s = launch_rotate_t<4>(c, st, p, eb, 2); break;
+    case 2: s = launch_rotate_t<2>(c, st, p, eb, 1); break;
+    default: s = launch_rotate_t<1>(c, st, p, eb, 0); break;
+    }
+    if (s != CYRSOXS_OK) return s;
     c->stats.stage_bytes[CYRSOXS_STAGE_ROTATE] += eb * (20.0 * c->Nx * c->Ny);
     return CYRSOXS_OK;
 }
@@ -325,16 +394,19 @@ cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int
         if ((s = launch_colpass(c, st, c->Ny, p, wz.W, F, pitch)) != CYRSOXS_OK) return s;
         c->stats.stage_bytes[CYRSOXS_STAGE_YPASS] += 8.0 * F * wz.W * pitch * ((double)c->Ny + wy.W);
     }
-    dim3 g2((c->Nx + 31) / 32, (c->Ny + 7) / 8, eb);
     {
         StageTimer t(c, st, CYRSOXS_STAGE_EWALD);
         EwaldParams p{};
         p.Nx = c->Nx; p.Ny = c->Ny; p.Nz = c->Nz; p.mode = c->ewald;
         p.dqx = c->dqx; p.dqy = c->dqy; p.dqz = c->dqz;
-        p.k = (const double *)c->d_k.p; p.e0 = e0;
+        p.k = (const double *)c->d_k.p; p.e0 = e0; p.n_e = eb;
         p.wx = wx; p.wy = wy; p.wz = wz; p.pitch = pitch;
         p.spec = A3; p.img = (float4 *)c->img.p;
-        k_ewald_chi<<<g2, 256, 0, st>>>(p);
+        switch (c->eg) {
+#define CASE(EG) case EG: k_ewald_chi<EG><<<ewald_grid<EG>(c, eb), 256, 0, st>>>(p); break;
+            CASE(8) CASE(4) CASE(2) default: CASE(1)
+#undef CASE
+        }
         CUDA_TRY(c, cudaGetLastError());
         const double nodes = (c->Nz > 1 && c->ewald == CYRSOXS_EWALD_TRILINEAR) ? 2.0 : 1.0;
         c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * 0.785 * nodes * NCHI * 8.0 + 16.0 * c->Nx * c->Ny);
@@ -453,18 +525,21 @@ cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &
 cyrsoxs_status run_batch_spectral(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, const Window &wx, const Window &wy,
                                   const Window &wz, int pitch, float *d_out, unsigned int *d_cnt)
 {
-    dim3 g2((c->Nx + 31) / 32, (c->Ny + 7) / 8, eb);
     {
         StageTimer t(c, st, CYRSOXS_STAGE_EWALD);
         EwaldBasisParams q{};
         EwaldParams &p = q.g;
         p.Nx = c->Nx; p.Ny = c->Ny; p.Nz = c->Nz; p.mode = c->ewald;
         p.dqx = c->dqx; p.dqy = c->dqy; p.dqz = c->dqz;
-        p.k = (const double *)c->d_k.p; p.e0 = e0;
+        p.k = (const double *)c->d_k.p; p.e0 = e0; p.n_e = eb;
         p.wx = wx; p.wy = wy; p.wz = wz; p.pitch = pitch;
         p.spec = (const float2 *)c->A3.p; p.img = (float4 *)c->img.p;
         q.n_pack = c->n_pack; q.coef = (const float2 *)c->d_bcoef.p; q.kind = (const int *)c->d_bkind.p;
-        k_ewald_basis<<<g2, 256, 0, st>>>(q);
+        switch (c->eg) {
+#define CASE(EG) case EG: k_ewald_basis<EG><<<ewald_grid<EG>(c, eb), 256, 0, st>>>(q); break;
+            CASE(8) CASE(4) CASE(2) default: CASE(1)
+#undef CASE
+        }
         CUDA_TRY(c, cudaGetLastError());
         const double nodes = (c->Nz > 1 && c->ewald == CYRSOXS_EWALD_TRILINEAR) ? 2.0 : 1.0;
         c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * 0.785 * nodes * 2.0 * c->n_pack * 8.0 + 16.0 * c->Nx * c->Ny);
@@ -515,7 +590,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
     if (!c) return;
     clear_prof(c);
     for (void *p : c->owned_morph) cudaFree(p);
-    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
+    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
                       &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind})
         release(*b);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
@@ -781,28 +856,38 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     const size_t per_img = sizeof(float4) * npix + (out_on_host ? 2 * sizeof(float) * npix : 0);
     const size_t per_e = spectral ? per_img : sizeof(float2) * (a1 + a2 + a3) + per_img;
     const size_t fixed = spectral ? sizeof(float2) * (a1 + a2 + a3) : 0;
-    size_t free_b = 0, total_b = 0;
-    CUDA_TRY(c, cudaMemGetInfo(&free_b, &total_b));
-    const size_t have = c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap;
-    const size_t budget = (size_t)((double)(free_b + have) * 0.85);
-    if (fixed + per_e > budget)
-        return fail(c, CYRSOXS_ERR_OOM, "workspace of %.1f GB does not fit in %.1f GB of free device memory",
-                    (double)(fixed + per_e) / 1e9, (double)budget / 1e9);
-    int eb = (int)std::min<size_t>((size_t)c->nE, std::max<size_t>(1, (budget - fixed) / per_e));
-    if (!spectral) {
-        // ~2 GiB of fields per batch is plenty of parallelism
-        const size_t target = (size_t)1 << 31;
-        eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / (sizeof(float2) * a1))));
-    } else {
-        const size_t target = (size_t)1 << 32;
-        eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / per_img)));
+    // The energy batch depends on the free device memory; cudaMemGetInfo is slow, so the batch is
+    // re-planned only when what it depends on has changed since the last run.
+    const unsigned long long plan_key = (unsigned long long)c->nE * 8 + (spectral ? 4 : 0) + (out_on_host ? 2 : 0) + 1;
+    int eb = c->plan_eb;
+    if (plan_key != c->plan_key || fixed != c->plan_fixed || per_e != c->plan_per_e || eb < 1) {
+        size_t free_b = 0, total_b = 0;
+        CUDA_TRY(c, cudaMemGetInfo(&free_b, &total_b));
+        const size_t have = c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap;
+        const size_t budget = (size_t)((double)(free_b + have) * 0.85);
+        if (fixed + per_e > budget)
+            return fail(c, CYRSOXS_ERR_OOM, "workspace of %.1f GB does not fit in %.1f GB of free device memory",
+                        (double)(fixed + per_e) / 1e9, (double)budget / 1e9);
+        eb = (int)std::min<size_t>((size_t)c->nE, std::max<size_t>(1, (budget - fixed) / per_e));
+        if (!spectral) {
+            // ~2 GiB of fields per batch is plenty of parallelism
+            const size_t target = (size_t)1 << 31;
+            eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / (sizeof(float2) * a1))));
+        } else {
+            const size_t target = (size_t)1 << 32;
+            eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / per_img)));
+        }
+        eb = std::min(eb, 256);
+        if (eb < c->nE && eb >= 8) eb = eb / 8 * 8;               // whole image groups in all but the last batch
+        c->plan_key = plan_key; c->plan_fixed = fixed; c->plan_per_e = per_e; c->plan_eb = eb;
     }
-    eb = std::min(eb, 256);
+    c->eg = choose_eg(eb);
+    const size_t eb_pad = (size_t)(eb + c->eg - 1) / c->eg * c->eg;
     const size_t mult = spectral ? 1 : (size_t)eb;
     if ((s = ensure(c, c->A1, sizeof(float2) * a1 * mult)) != CYRSOXS_OK) return s;
     if (a2 && (s = ensure(c, c->A2, sizeof(float2) * a2 * mult)) != CYRSOXS_OK) return s;
     if ((s = ensure(c, c->A3, sizeof(float2) * a3 * mult)) != CYRSOXS_OK) return s;
-    if ((s = ensure(c, c->img, sizeof(float4) * npix * eb)) != CYRSOXS_OK) return s;
+    if ((s = ensure(c, c->img, sizeof(float4) * npix * eb_pad)) != CYRSOXS_OK) return s;
     if (out_on_host) {
         for (int i = 0; i < 2; ++i)
             if ((s = ensure(c, c->stage_out[i], sizeof(float) * npix * eb)) != CYRSOXS_OK) return s;
@@ -871,8 +956,10 @@ cyrsoxs_status cyrsoxs_debug_fetch_images(cyrsoxs_ctx *c, int e_in_batch, float 
     if (!c || !d_dst) return CYRSOXS_ERR_INVALID_ARG;
     if (!c->img.p || e_in_batch < 0 || e_in_batch >= c->last_batch_e) return fail(c, CYRSOXS_ERR_INVALID_ARG, "no such image");
     const size_t npix = (size_t)c->Nx * c->Ny;
-    CUDA_TRY(c, cudaMemcpyAsync(d_dst, (const float4 *)c->img.p + (size_t)e_in_batch * npix, sizeof(float4) * npix,
-                                cudaMemcpyDeviceToDevice, c->last_stream));
+    const int eg = c->eg;
+    const float4 *src = (const float4 *)c->img.p + (size_t)(e_in_batch / eg) * npix * eg + e_in_batch % eg;
+    CUDA_TRY(c, cudaMemcpy2DAsync(d_dst, sizeof(float4), src, sizeof(float4) * eg, sizeof(float4), npix,
+                                  cudaMemcpyDeviceToDevice, c->last_stream));
     return CYRSOXS_OK;
 }
 

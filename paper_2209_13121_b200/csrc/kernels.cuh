@@ -346,15 +346,24 @@ k_colpass(const ColParams p)
 
 // ------------------------------------------------------------------------------------------
 // Ewald projection.  One thread per detector pixel and energy.
+// Image layout shared by the Ewald and rotate kernels ("energy interleaved"): the batch's
+// energies are grouped EG at a time (EG = 1, 2, 4 or 8) and the float4 of energy e at pixel
+// (iy, ix) sits at  img[(((e / EG) * Ny + iy) * Nx + ix) * EG + e % EG].
+// Lanes of a warp run over the EG energies of a group first and over 32 / EG adjacent pixels
+// second: the bilinear taps of the rotate kernel, whose position depends on the pixel and the
+// angle but not on the energy, then fetch EG * 16 contiguous bytes per pixel (one full 128-byte
+// line for EG = 8) instead of 16 bytes from 32 scattered places -- ncu showed that kernel bound
+// by L1 wavefronts (14 per 128-bit load, profiles/r1b) -- and the Ewald kernels read the
+// spectrum once per pixel for EG energies (same address across the EG lanes: a broadcast).
 struct EwaldParams {
     int Nx, Ny, Nz, mode;
     double dqx, dqy, dqz;
     const double *k;            // [n_energy] wavenumbers, nm^-1
-    int e0;
+    int e0, n_e;                // first energy of the batch, energies in the batch
     Window wx, wy, wz;
     int pitch;                  // x pitch of the spectrum cube
     const float2 *spec;         // [e][f][slot_z][slot_y][pitch]
-    float4 *img;                // [e][Ny][Nx]  (I_xx, I_yy, I_xy, valid)
+    float4 *img;                // energy-interleaved (I_xx, I_yy, I_xy, valid)
 };
 
 struct PixelGeom {
@@ -414,39 +423,52 @@ __device__ __forceinline__ void project_pair(const float r[3], const float2 u[3]
     }
 }
 
+// Thread mapping of both Ewald kernels: 256 threads = 256 / EG pixels x EG energies.
+template <int EG> struct EwaldMap {
+    static constexpr int P = 256 / EG;                 // pixels per CTA
+    static constexpr int PW = P >= 32 ? 32 : P;        // ... as PW x PH
+    static constexpr int PH = P / PW;
+};
+
+template <int EG>
 __global__ void __launch_bounds__(256)
 k_ewald_chi(const EwaldParams p)
 {
-    const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
-    const int iy = blockIdx.y * 8 + (threadIdx.x >> 5);
-    const int e = blockIdx.z;
+    using M = EwaldMap<EG>;
+    const int sub = threadIdx.x % EG, pp = threadIdx.x / EG;
+    const int ix = blockIdx.x * M::PW + pp % M::PW;
+    const int iy = blockIdx.y * M::PH + pp / M::PW;
+    const int e = blockIdx.z * EG + sub;
     if (ix >= p.Nx || iy >= p.Ny) return;
-    const double k = p.k[p.e0 + e];
-    const PixelGeom g = pixel_geometry(ix, iy, p.Nx, p.Ny, p.Nz, p.mode, p.dqx, p.dqy, p.dqz, k);
     float axx = 0.f, ayy = 0.f, axy = 0.f;
-    bool valid = g.n_nodes > 0;
-    if (valid) {
-        const int sx = win_slot(p.wx, ix - p.Nx / 2), sy = win_slot(p.wy, iy - p.Ny / 2);
-        const size_t plane = (size_t)p.wy.W * p.pitch;
-        const size_t fstride = plane * p.wz.W;
-        const float2 *base = p.spec + (size_t)e * NCHI * fstride + (size_t)sy * p.pitch + sx;
-        const double k2 = k * k;
-        const float k4 = (float)(k2 * k2);
-        const bool inwin = sx < p.wx.W && sy < p.wy.W;
-        for (int j = 0; j < g.n_nodes; ++j) {
-            const int sz = win_slot(p.wz, g.node[j]);
-            float2 c[NCHI];
+    bool valid = false;
+    if (e < p.n_e) {
+        const double k = p.k[p.e0 + e];
+        const PixelGeom g = pixel_geometry(ix, iy, p.Nx, p.Ny, p.Nz, p.mode, p.dqx, p.dqy, p.dqz, k);
+        valid = g.n_nodes > 0;
+        if (valid) {
+            const int sx = win_slot(p.wx, ix - p.Nx / 2), sy = win_slot(p.wy, iy - p.Ny / 2);
+            const size_t plane = (size_t)p.wy.W * p.pitch;
+            const size_t fstride = plane * p.wz.W;
+            const float2 *base = p.spec + (size_t)e * NCHI * fstride + (size_t)sy * p.pitch + sx;
+            const double k2 = k * k;
+            const float k4 = (float)(k2 * k2);
+            const bool inwin = sx < p.wx.W && sy < p.wy.W;
+            for (int j = 0; j < g.n_nodes; ++j) {
+                const int sz = win_slot(p.wz, g.node[j]);
+                float2 c[NCHI];
 #pragma unroll
-            for (int f = 0; f < NCHI; ++f)
-                c[f] = (inwin && sz < p.wz.W) ? __ldg(base + f * fstride + (size_t)sz * plane) : make_float2(0.f, 0.f);
-            const float2 u[3] = {c[0], c[1], c[2]}, v[3] = {c[1], c[3], c[4]};
-            float sxx, syy, sxy;
-            project_pair(g.r, u, v, sxx, syy, sxy);
-            const float w = g.wt[j] * k4;
-            axx = fmaf(w, sxx, axx); ayy = fmaf(w, syy, ayy); axy = fmaf(w, sxy, axy);
+                for (int f = 0; f < NCHI; ++f)
+                    c[f] = (inwin && sz < p.wz.W) ? __ldg(base + f * fstride + (size_t)sz * plane) : make_float2(0.f, 0.f);
+                const float2 u[3] = {c[0], c[1], c[2]}, v[3] = {c[1], c[3], c[4]};
+                float sxx, syy, sxy;
+                project_pair(g.r, u, v, sxx, syy, sxy);
+                const float w = g.wt[j] * k4;
+                axx = fmaf(w, sxx, axx); ayy = fmaf(w, syy, ayy); axy = fmaf(w, sxy, axy);
+            }
         }
     }
-    p.img[((size_t)e * p.Ny + iy) * p.Nx + ix] = make_float4(axx, ayy, axy, valid ? 1.f : 0.f);
+    p.img[(((size_t)blockIdx.z * p.Ny + iy) * p.Nx + ix) * EG + sub] = make_float4(axx, ayy, axy, valid ? 1.f : 0.f);
 }
 
 // Ewald projection for SPECTRAL_BASIS: chi~(q) = sum_b coef[e][b] F_b(q) on the shell only.
@@ -457,76 +479,97 @@ struct EwaldBasisParams {
     const int *kind;            // [2 n_pack] BasisKind
 };
 
+template <int EG>
 __global__ void __launch_bounds__(256)
 k_ewald_basis(const EwaldBasisParams q)
 {
+    using M = EwaldMap<EG>;
     const EwaldParams &p = q.g;
-    const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
-    const int iy = blockIdx.y * 8 + (threadIdx.x >> 5);
-    const int e = blockIdx.z;
+    const int sub = threadIdx.x % EG, pp = threadIdx.x / EG;
+    const int ix = blockIdx.x * M::PW + pp % M::PW;
+    const int iy = blockIdx.y * M::PH + pp / M::PW;
+    const int e = blockIdx.z * EG + sub;
     if (ix >= p.Nx || iy >= p.Ny) return;
-    const double k = p.k[p.e0 + e];
-    const PixelGeom g = pixel_geometry(ix, iy, p.Nx, p.Ny, p.Nz, p.mode, p.dqx, p.dqy, p.dqz, k);
     float axx = 0.f, ayy = 0.f, axy = 0.f;
-    const bool valid = g.n_nodes > 0;
-    if (valid) {
-        const int mx = ix - p.Nx / 2, my = iy - p.Ny / 2;
-        const int sx = win_slot(p.wx, mx), sy = win_slot(p.wy, my);
-        const int tx = win_slot(p.wx, -mx), ty = win_slot(p.wy, -my);
-        const size_t plane = (size_t)p.wy.W * p.pitch;
-        const size_t fstride = plane * p.wz.W;
-        const bool inwin = sx < p.wx.W && sy < p.wy.W && tx < p.wx.W && ty < p.wy.W;
-        const double k2 = k * k;
-        const float k4 = (float)(k2 * k2);
-        const float2 *coef = q.coef + (size_t)(p.e0 + e) * 2 * q.n_pack;
-        for (int j = 0; j < g.n_nodes; ++j) {
-            const int sz = win_slot(p.wz, g.node[j]), tz = win_slot(p.wz, -g.node[j]);
-            const bool ok = inwin && sz < p.wz.W && tz < p.wz.W;
-            const float2 *pq = p.spec + (size_t)sz * plane + (size_t)sy * p.pitch + sx;
-            const float2 *pm = p.spec + (size_t)tz * plane + (size_t)ty * p.pitch + tx;
-            float2 c[NCHI];
+    bool valid = false;
+    if (e < p.n_e) {
+        const double k = p.k[p.e0 + e];
+        const PixelGeom g = pixel_geometry(ix, iy, p.Nx, p.Ny, p.Nz, p.mode, p.dqx, p.dqy, p.dqz, k);
+        valid = g.n_nodes > 0;
+        if (valid) {
+            const int mx = ix - p.Nx / 2, my = iy - p.Ny / 2;
+            const int sx = win_slot(p.wx, mx), sy = win_slot(p.wy, my);
+            const int tx = win_slot(p.wx, -mx), ty = win_slot(p.wy, -my);
+            const size_t plane = (size_t)p.wy.W * p.pitch;
+            const size_t fstride = plane * p.wz.W;
+            const bool inwin = sx < p.wx.W && sy < p.wy.W && tx < p.wx.W && ty < p.wy.W;
+            const double k2 = k * k;
+            const float k4 = (float)(k2 * k2);
+            const float2 *coef = q.coef + (size_t)(p.e0 + e) * 2 * q.n_pack;
+            for (int j = 0; j < g.n_nodes; ++j) {
+                const int sz = win_slot(p.wz, g.node[j]), tz = win_slot(p.wz, -g.node[j]);
+                const bool ok = inwin && sz < p.wz.W && tz < p.wz.W;
+                const float2 *pq = p.spec + (size_t)sz * plane + (size_t)sy * p.pitch + sx;
+                const float2 *pm = p.spec + (size_t)tz * plane + (size_t)ty * p.pitch + tx;
+                float2 c[NCHI];
 #pragma unroll
-            for (int f = 0; f < NCHI; ++f) c[f] = make_float2(0.f, 0.f);
-            for (int pk = 0; ok && pk < q.n_pack; ++pk) {
-                const float2 z1 = __ldg(pq + pk * fstride), z2 = __ldg(pm + pk * fstride);
-                // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
-                const float2 F[2] = {make_float2(z1.x + z2.x, z1.y - z2.y), make_float2(z1.y + z2.y, z2.x - z1.x)};
+                for (int f = 0; f < NCHI; ++f) c[f] = make_float2(0.f, 0.f);
+                for (int pk = 0; ok && pk < q.n_pack; ++pk) {
+                    const float2 z1 = __ldg(pq + pk * fstride), z2 = __ldg(pm + pk * fstride);
+                    // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
+                    const float2 F[2] = {make_float2(z1.x + z2.x, z1.y - z2.y), make_float2(z1.y + z2.y, z2.x - z1.x)};
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int kd = __ldg(q.kind + 2 * pk + h);
-                    const float2 v = cmul(__ldg(coef + 2 * pk + h), F[h]);
-                    if (kd == BK_PHI || kd == BK_W) { c[0] = cadd(c[0], v); c[3] = cadd(c[3], v); }
-                    else if (kd == BK_XX) c[0] = cadd(c[0], v);
-                    else if (kd == BK_YY) c[3] = cadd(c[3], v);
-                    else if (kd == BK_XY) c[1] = cadd(c[1], v);
-                    else if (kd == BK_XZ) c[2] = cadd(c[2], v);
-                    else if (kd == BK_YZ) c[4] = cadd(c[4], v);
+                    for (int h = 0; h < 2; ++h) {
+                        const int kd = __ldg(q.kind + 2 * pk + h);
+                        const float2 v = cmul(__ldg(coef + 2 * pk + h), F[h]);
+                        if (kd == BK_PHI || kd == BK_W) { c[0] = cadd(c[0], v); c[3] = cadd(c[3], v); }
+                        else if (kd == BK_XX) c[0] = cadd(c[0], v);
+                        else if (kd == BK_YY) c[3] = cadd(c[3], v);
+                        else if (kd == BK_XY) c[1] = cadd(c[1], v);
+                        else if (kd == BK_XZ) c[2] = cadd(c[2], v);
+                        else if (kd == BK_YZ) c[4] = cadd(c[4], v);
+                    }
                 }
+                const float2 u[3] = {c[0], c[1], c[2]}, v[3] = {c[1], c[3], c[4]};
+                float sxx, syy, sxy;
+                project_pair(g.r, u, v, sxx, syy, sxy);
+                const float w = g.wt[j] * k4;
+                axx = fmaf(w, sxx, axx); ayy = fmaf(w, syy, ayy); axy = fmaf(w, sxy, axy);
             }
-            const float2 u[3] = {c[0], c[1], c[2]}, v[3] = {c[1], c[3], c[4]};
-            float sxx, syy, sxy;
-            project_pair(g.r, u, v, sxx, syy, sxy);
-            const float w = g.wt[j] * k4;
-            axx = fmaf(w, sxx, axx); ayy = fmaf(w, syy, ayy); axy = fmaf(w, sxy, axy);
         }
     }
-    p.img[((size_t)e * p.Ny + iy) * p.Nx + ix] = make_float4(axx, ayy, axy, valid ? 1.f : 0.f);
+    p.img[(((size_t)blockIdx.z * p.Ny + iy) * p.Nx + ix) * EG + sub] = make_float4(axx, ayy, axy, valid ? 1.f : 0.f);
 }
 
 // ------------------------------------------------------------------------------------------
-// Rotate back and average (DESIGN 3-A9/A10).  One thread per output pixel and EPT energies:
-// the bilinear cell of an (output pixel, angle) pair is pure geometry (fp64, every operation
-// rounded on its own) and does not depend on the energy, so it is computed once and reused for
-// the EPT images the thread accumulates.  cs[a] = (C, S) in double; csf[a] = (C^2, S^2, 2 C S).
+// Rotate back and average (DESIGN 3-A9/A10).  A thread owns one output pixel and one energy of
+// every energy group (lanes: EG energies x 32/EG pixels, see EwaldParams).  The bilinear cell
+// of an (output pixel, angle) pair is pure geometry (fp64, every operation rounded on its own)
+// and does not depend on the energy: it is computed once per angle and reused for all groups.
+// cs[a] = (C, S) in double; csf[a] = (C^2, S^2, 2 C S).
+//  * tiles are visited in order of their distance from q = 0 (table built on the host): the CTAs
+//    resident at one time cover an annulus, and the source pixels of an annulus are the same
+//    annulus at every angle, so an image is read from DRAM about once instead of once per angle;
+//  * all 4 UA loads of an angle chunk are issued before the first use.
 struct RotateParams {
     int Nx, Ny, n_angles, n_energy;
     const double2 *cs;
     const float4 *csf;
-    const float4 *img;          // [e][Ny][Nx]
+    const float4 *img;          // energy-interleaved, see EwaldParams
     float *out;                 // [e][Ny][Nx]
     unsigned int *counts;       // optional
     const float *reach2;        // [e] squared reach (in pixels of x) of the valid disk, see below
+    const uint32_t *tiles;      // [n_tiles] (tile_y << 16 | tile_x), sorted by distance from q = 0
     double rho;                 // Nx / Ny
+    int gpc;                    // energy groups per CTA (blockIdx.y slices the groups)
+};
+
+// 256 threads: 8 warps as 4 (x) by 2 (y); a warp covers WPW x WPH pixels times EG energies.
+template <int EG> struct RotMap {
+    static constexpr int WP = 32 / EG;                                        // pixels per warp
+    static constexpr int WPW = WP >= 16 ? 8 : (WP == 8 ? 4 : 2);              // 8x4, 8x2, 4x2, 2x2
+    static constexpr int WPH = WP / WPW;
+    static constexpr int TW = 4 * WPW, TH = 2 * WPH;                          // CTA tile
 };
 
 // reach2[e] = (k_e/dq_x + 3)^2: an output pixel whose distance from q = 0 (measured in x
@@ -534,68 +577,102 @@ struct RotateParams {
 // Ewald disk s^2 >= 0 at every angle (rotation keeps the distance, a cell adds < 2 pixels), so
 // its count is 0 and nothing needs to be read.  The margin of 3 keeps the decision away from
 // rounding: only pixels that are invalid with certainty are skipped.
-template <int EPT>
-__global__ void __launch_bounds__(128)
+//
+// Loop order: angles in chunks of UA; the chunk's cells are computed once (registers) and
+// then applied to every energy group of the CTA's slice (blockIdx.y, gpc <= ROT_GMAX groups),
+// whose running sums and counts live in shared memory between chunks.
+constexpr int ROT_GMAX = 16;      // most energy groups per CTA (RotateParams::gpc <= ROT_GMAX)
+
+template <int EG, int UA, int MINB>
+__global__ void __launch_bounds__(256, MINB)
 k_rotate_avg(const RotateParams p)
 {
-    const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
-    const int iy = blockIdx.y * 4 + (threadIdx.x >> 5);
-    const int e0 = blockIdx.z * EPT;
-    if (ix >= p.Nx || iy >= p.Ny) return;
-    const size_t plane = (size_t)p.Ny * p.Nx;
-    const float4 *img = p.img + (size_t)e0 * plane;
-    const int ne = min(EPT, p.n_energy - e0);
+    using M = RotMap<EG>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int n_groups = (p.n_energy + EG - 1) / EG;
+    const int g0 = blockIdx.y * p.gpc;
+    const int ng = min(min(p.gpc, ROT_GMAX), n_groups - g0);
+    float *s_sum = reinterpret_cast<float *>(smem_raw);                       // [ng][256]
+    unsigned int *s_cnt = reinterpret_cast<unsigned int *>(s_sum + ng * 256);  // [ng][256]
+    const uint32_t tile = __ldg(p.tiles + blockIdx.x);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int sub = lane % EG, lp = lane / EG;
+    const int ix = (int)(tile & 0xffffu) * M::TW + (warp & 3) * M::WPW + lp % M::WPW;
+    const int iy = (int)(tile >> 16) * M::TH + (warp >> 2) * M::WPH + lp / M::WPW;
+    if (ix >= p.Nx || iy >= p.Ny) return;                       // no block-wide barrier below
+    const size_t plane = (size_t)p.Ny * p.Nx * EG;               // float4 per energy group
+    const float4 *img = p.img + (size_t)g0 * plane + sub;
     const double rho = p.rho;
     const double u = (double)(ix - p.Nx / 2), v = (double)(iy - p.Ny / 2);
     const double vr = v * rho, ur = u / rho;                 // exact: rho is a power of two
     const double cx = (double)(p.Nx / 2), cy = (double)(p.Ny / 2);
+    const double xmax = (double)(p.Nx - 1), ymax = (double)(p.Ny - 1);
     const float r2 = (float)(u * u + vr * vr);
-    float sum[EPT];
-    unsigned int cnt[EPT];
-    bool live[EPT];
-    bool any = false;
-#pragma unroll
-    for (int j = 0; j < EPT; ++j) {
-        sum[j] = 0.f; cnt[j] = 0;
-        live[j] = j < ne && r2 <= __ldg(p.reach2 + e0 + j);
-        any |= live[j];
+    // live groups of this lane: bit j <=> energy (g0 + j) EG + sub exists and the pixel is within its reach
+    unsigned int live = 0;
+    for (int j = 0; j < ng; ++j) {
+        const int e = (g0 + j) * EG + sub;
+        if (e < p.n_energy && r2 <= __ldg(p.reach2 + e)) live |= 1u << j;
+        s_sum[j * 256 + tid] = 0.f;
+        s_cnt[j * 256 + tid] = 0u;
     }
-    for (int a = 0; any && a < p.n_angles; ++a) {
-        const double2 cs = p.cs[a];
-        const double fx = __dadd_rn(__dsub_rn(__dmul_rn(cs.x, u), __dmul_rn(cs.y, vr)), cx);
-        const double fy = __dadd_rn(__dadd_rn(__dmul_rn(cs.y, ur), __dmul_rn(cs.x, v)), cy);
-        const double x0 = floor(fx), y0 = floor(fy);
-        const double al = fx - x0, be = fy - y0;
-        const int dx = al > 0.0 ? 1 : 0, dy = be > 0.0 ? 1 : 0;    // a neighbour is needed iff its weight > 0
-        if (x0 < 0.0 || y0 < 0.0 || x0 + (double)dx > (double)(p.Nx - 1) || y0 + (double)dy > (double)(p.Ny - 1))
-            continue;
-        const int X0 = (int)x0, Y0 = (int)y0;
-        const float4 w = p.csf[a];
-        const float fa = (float)al, fb = (float)be;
-        const float w00 = (1.f - fa) * (1.f - fb), w10 = fa * (1.f - fb), w01 = (1.f - fa) * fb, w11 = fa * fb;
-        // un-needed neighbours alias a needed one (weight 0, same validity)
-        const float4 *p00 = img + (size_t)Y0 * p.Nx + X0;
-        const float4 *p10 = p00 + dx, *p01 = p00 + (size_t)dy * p.Nx, *p11 = p01 + dx;
+    const int na = live ? p.n_angles : 0;
+    const int rowq = p.Nx * EG;
+    for (int a0 = 0; a0 < na; a0 += UA) {
+        int o00[UA], ox[UA], oy[UA];
+        float w00[UA], w10[UA], w01[UA], w11[UA], wx[UA], wy[UA], wz[UA];
+        bool ok[UA];
 #pragma unroll
-        for (int j = 0; j < EPT; ++j) {
-            if (live[j]) {
-                const float4 t00 = __ldg(p00 + j * plane), t10 = __ldg(p10 + j * plane);
-                const float4 t01 = __ldg(p01 + j * plane), t11 = __ldg(p11 + j * plane);
-                const bool ok = (t00.w != 0.f) & (t10.w != 0.f) & (t01.w != 0.f) & (t11.w != 0.f);
-                float acc = w00 * (w.x * t00.x + w.y * t00.y + w.z * t00.z);
-                acc = fmaf(w10, w.x * t10.x + w.y * t10.y + w.z * t10.z, acc);
-                acc = fmaf(w01, w.x * t01.x + w.y * t01.y + w.z * t01.z, acc);
-                acc = fmaf(w11, w.x * t11.x + w.y * t11.y + w.z * t11.z, acc);
-                if (ok) { sum[j] += acc; ++cnt[j]; }
+        for (int q = 0; q < UA; ++q) {
+            const int a = min(a0 + q, na - 1);
+            const double2 cs = __ldg(p.cs + a);
+            const float4 w = __ldg(p.csf + a);
+            wx[q] = w.x; wy[q] = w.y; wz[q] = w.z;
+            const double fx = __dadd_rn(__dsub_rn(__dmul_rn(cs.x, u), __dmul_rn(cs.y, vr)), cx);
+            const double fy = __dadd_rn(__dadd_rn(__dmul_rn(cs.y, ur), __dmul_rn(cs.x, v)), cy);
+            const double x0 = floor(fx), y0 = floor(fy);
+            const double al = fx - x0, be = fy - y0;
+            const int dx = al > 0.0 ? 1 : 0, dy = be > 0.0 ? 1 : 0;    // a neighbour is needed iff its weight > 0
+            ok[q] = (a0 + q < na) && !(x0 < 0.0 || y0 < 0.0 || x0 + (double)dx > xmax || y0 + (double)dy > ymax);
+            // un-needed neighbours alias a needed one (weight 0, same validity)
+            o00[q] = ok[q] ? ((int)y0 * p.Nx + (int)x0) * EG : 0;
+            ox[q] = ok[q] ? dx * EG : 0; oy[q] = ok[q] ? dy * rowq : 0;
+            const float fa = (float)al, fb = (float)be;
+            w00[q] = (1.f - fa) * (1.f - fb); w10[q] = fa * (1.f - fb); w01[q] = (1.f - fa) * fb; w11[q] = fa * fb;
+        }
+        for (int j = 0; j < ng; ++j) {
+            if (!((live >> j) & 1u)) continue;
+            const float4 *base = img + (size_t)j * plane;
+            float4 t[UA][4];
+#pragma unroll
+            for (int q = 0; q < UA; ++q) {
+                const float4 *p00 = base + o00[q];
+                t[q][0] = __ldg(p00); t[q][1] = __ldg(p00 + ox[q]);
+                t[q][2] = __ldg(p00 + oy[q]); t[q][3] = __ldg(p00 + oy[q] + ox[q]);
             }
+            float sum = s_sum[j * 256 + tid];
+            unsigned int cnt = s_cnt[j * 256 + tid];
+#pragma unroll
+            for (int q = 0; q < UA; ++q) {
+                const float4 t00 = t[q][0], t10 = t[q][1], t01 = t[q][2], t11 = t[q][3];
+                const bool good = ok[q] & (t00.w != 0.f) & (t10.w != 0.f) & (t01.w != 0.f) & (t11.w != 0.f);
+                float acc = w00[q] * (wx[q] * t00.x + wy[q] * t00.y + wz[q] * t00.z);
+                acc = fmaf(w10[q], wx[q] * t10.x + wy[q] * t10.y + wz[q] * t10.z, acc);
+                acc = fmaf(w01[q], wx[q] * t01.x + wy[q] * t01.y + wz[q] * t01.z, acc);
+                acc = fmaf(w11[q], wx[q] * t11.x + wy[q] * t11.y + wz[q] * t11.z, acc);
+                if (good) { sum += acc; ++cnt; }
+            }
+            s_sum[j * 256 + tid] = sum;
+            s_cnt[j * 256 + tid] = cnt;
         }
     }
-#pragma unroll
-    for (int j = 0; j < EPT; ++j) {
-        if (j < ne) {
-            const size_t o = ((size_t)(e0 + j) * p.Ny + iy) * p.Nx + ix;
-            p.out[o] = cnt[j] ? sum[j] / (float)cnt[j] : 0.f;
-            if (p.counts) p.counts[o] = cnt[j];
+    for (int j = 0; j < ng; ++j) {
+        const int e = (g0 + j) * EG + sub;
+        if (e < p.n_energy) {
+            const size_t o = ((size_t)e * p.Ny + iy) * p.Nx + ix;
+            const unsigned int cnt = s_cnt[j * 256 + tid];
+            p.out[o] = cnt ? s_sum[j * 256 + tid] / (float)cnt : 0.f;
+            if (p.counts) p.counts[o] = cnt;
         }
     }
 }
