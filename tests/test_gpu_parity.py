@@ -1,5 +1,7 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded
 inputs, element by element, with the north_star gates (tests/parity.py)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -84,6 +86,58 @@ def test_cfg4_reduced(alg):
     ref, rcnt = oracle_run(w, linear=True)
     out, cnt, _ = _gpu(w, alg)
     print("cfg4/256", compare(out, cnt, ref, rcnt, "cfg4/256"))
+
+
+def _full_size_sampled(w, energy_idx, label):
+    """Full-size config through the launch configuration bench.py uses (AUTO algorithm, all
+    energies in one run); the oracle (linear mode) recomputes the sampled energies one by one."""
+    out, cnt, ctx = _gpu(w, 0)
+    assert np.isfinite(out).all()
+    st = ctx.stats()
+    for e in energy_idx:
+        w1 = w.restrict_energies([e])
+        ref, rcnt = oracle_run(w1, linear=True)
+        r = compare(out[e:e + 1], cnt[e:e + 1], ref, rcnt, f"{label} e={e}")
+        print(label, "energy", e, r, "algorithm", st["algorithm"], "batch", st["energy_batch"])
+
+
+def test_cfg3_full_size_sampled_energies():
+    """BASELINE configs[2] at full size (512x512x256, 50 energies, trilinear): first, middle and
+    last energy (largest k: the one that sizes the spectral windows) against the oracle."""
+    w = W.cfg3()
+    _full_size_sampled(w, [0, 24, 49], "cfg3")
+
+
+def test_cfg4_full_size_sampled_energies():
+    """BASELINE configs[3] at full size (2048x2048x1, 4 materials, 100 energies x 36 angles)."""
+    w = W.cfg4()
+    _full_size_sampled(w, [0, 63, 64, 99], "cfg4")      # 63/64 straddle the energy-batch boundary
+
+
+def _host_ram_gb():
+    try:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable"):
+                return int(line.split()[1]) / 1e6
+    except OSError:
+        pass
+    return 0.0
+
+
+def test_cfg5_quarter_depth_sampled_energies():
+    """BASELINE configs[4] at full lateral size and a quarter of the depth (1024x1024x128, 1.3e8
+    voxels; same generator, same energies, trilinear).  The full-depth run is the next test."""
+    w = W.cfg5(nz=128)
+    _full_size_sampled(w, [0, 19], "cfg5/nz128")
+
+
+@pytest.mark.skipif(_host_ram_gb() < 100.0 or os.environ.get("CYRSOXS_SKIP_FULL_CFG5") == "1",
+                    reason="full CFG5 needs ~90 GB of host RAM for the generator and the oracle (about 80 s on the B200 box)")
+def test_cfg5_full_size_sampled_energy():
+    """BASELINE configs[4] at full size (1024x1024x512 = 5.4e8 voxels, 17 GB of morphology):
+    64-bit indexing, memory footprint, the largest windows."""
+    w = W.cfg5()
+    _full_size_sampled(w, [19], "cfg5")
 
 
 @pytest.mark.parametrize("alg", ALGS)
