@@ -246,3 +246,16 @@ def run(materials, voxel_nm, energies_eV, delta_par, beta_par, delta_perp, beta_
     if imgs is not None:
         return out, cnt, imgs
     return out, cnt
+
+
+def reductions(img, cnt, voxel_nm, n_bins, sector_half_width_deg=20.0):
+    """NEXT-1 reductions of one image [Ny][Nx]: (I[n_bins], A[n_bins], npix[n_bins], ISI).
+    cnt may be None (every pixel takes part)."""
+    img = np.ascontiguousarray(img, np.float64)
+    Ny, Nx = img.shape
+    c = None if cnt is None else np.ascontiguousarray(cnt, np.uint32)
+    I = np.zeros(n_bins); A = np.zeros(n_bins); npix = np.zeros(n_bins, np.uint32); isi = C.c_double(0.0)
+    tan_w = float(np.tan(np.deg2rad(np.float64(sector_half_width_deg))))
+    lib().orc_reductions(C.c_int(Nx), C.c_int(Ny), C.c_double(voxel_nm), _p(img), None if c is None else _p(c),
+                         C.c_int(n_bins), C.c_double(tan_w), _p(I), _p(A), _p(npix), C.byref(isi))
+    return I, A, npix, isi.value
