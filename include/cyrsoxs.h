@@ -154,6 +154,24 @@ int cyrsoxs_num_angles(const cyrsoxs_ctx *ctx);
  * profiling is enabled. */
 cyrsoxs_status cyrsoxs_get_stats(cyrsoxs_ctx *ctx, cyrsoxs_stats *stats);
 
+/* 1-D reductions of finished images (the quantities of the paper's
+ * validation figures: azimuthal average I(|q|) Fig. 5b/8b P:387 P:415, scattering anisotropy
+ * Fig. 15, integrated scattering intensity Fig. 6 / Eq. 10).  The paper gives no
+ * binning rule; DESIGN.md 12 fixes one.  For each of the n_energy images d_images[e][Ny][Nx]
+ * (DEVICE, e.g. the `out` of cyrsoxs_run) and with u = ix - Nx/2, v = (iy - Ny/2) Nx/Ny:
+ *   radial bin b = floor(sqrt(u^2 + v^2) + 1/2), kept if b < n_bins (|q| = b dq_x);
+ *   only pixels with d_counts[e][iy][ix] > 0 take part (d_counts NULL: all pixels);
+ *   d_I[e][b]    mean over the bin's pixels (0 if none);
+ *   d_A[e][b]    (I_para - I_perp)/(I_para + I_perp), sector means over the bin's pixels within
+ *                sector_half_width_deg of the q_x axis (para: the E-field axis after the
+ *                rotate-back step) resp. of the q_y axis; 0 if a sector is empty;
+ *   d_isi[e]     dq_x dq_y times the sum over ALL valid pixels of the image.
+ * All outputs are float32 in DEVICE memory (d_A and d_isi may be NULL); sums are accumulated in
+ * double.  1 <= n_bins <= 4096, 0 < sector_half_width_deg <= 45.  Enqueued on cuda_stream. */
+cyrsoxs_status cyrsoxs_reduce(cyrsoxs_ctx *ctx, void *cuda_stream, const float *d_images,
+                              const unsigned int *d_counts, int n_energy, int n_bins,
+                              double sector_half_width_deg, float *d_I, float *d_A, float *d_isi);
+
 /* Test hook, not part of the contract: copies the per-energy Ewald images of the LAST energy
  * batch of the last run, as float4 (I_xx, I_yy, I_xy, valid) per pixel, for batch-local energy
  * index `e_in_batch`, into d_dst (Ny*Nx*4 floats, device).  Enqueued on the run's stream. */

@@ -22,7 +22,7 @@ EXPORTS = [
     "cyrsoxs_create", "cyrsoxs_set_morphology", "cyrsoxs_set_morphology_host",
     "cyrsoxs_set_optical_constants", "cyrsoxs_set_angles", "cyrsoxs_set_ewald", "cyrsoxs_set_algorithm",
     "cyrsoxs_set_counts_output", "cyrsoxs_set_profiling", "cyrsoxs_run", "cyrsoxs_num_angles",
-    "cyrsoxs_get_stats", "cyrsoxs_debug_fetch_images", "cyrsoxs_last_error", "cyrsoxs_destroy",
+    "cyrsoxs_get_stats", "cyrsoxs_reduce", "cyrsoxs_debug_fetch_images", "cyrsoxs_last_error", "cyrsoxs_destroy",
     "cyrsoxs_version",
 ]
 
@@ -68,6 +68,7 @@ def load() -> C.CDLL:
     lib.cyrsoxs_num_angles.argtypes = [vp]
     lib.cyrsoxs_get_stats.argtypes = [vp, C.POINTER(Stats)]
     lib.cyrsoxs_debug_fetch_images.argtypes = [vp, C.c_int, vp]
+    lib.cyrsoxs_reduce.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, C.c_double, vp, vp, vp]
     lib.cyrsoxs_last_error.argtypes = [vp]
     lib.cyrsoxs_last_error.restype = C.c_char_p
     lib.cyrsoxs_destroy.argtypes = [vp]
@@ -192,6 +193,11 @@ class Context:
             "stage_ms": {n: float(s.stage_ms[i]) for i, n in enumerate(STAGES)},
             "workspace_bytes": float(s.workspace_bytes),
         }
+
+    def reduce(self, images_ptr: int, counts_ptr: Optional[int], n_energy: int, n_bins: int, sector_half_width_deg: float,
+               I_ptr: int, A_ptr: Optional[int] = None, isi_ptr: Optional[int] = None, stream: int = 0):
+        self._check(self.lib.cyrsoxs_reduce(self.h, stream or None, images_ptr, counts_ptr or None, n_energy, n_bins,
+                                            float(sector_half_width_deg), I_ptr, A_ptr or None, isi_ptr or None))
 
     def debug_fetch_images(self, e_in_batch: int, dst_ptr: int):
         self._check(self.lib.cyrsoxs_debug_fetch_images(self.h, e_in_batch, C.c_void_p(dst_ptr)))

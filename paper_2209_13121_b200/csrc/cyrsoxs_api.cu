@@ -17,6 +17,7 @@
 #include "../../include/cyrsoxs.h"
 #include "kernels.cuh"
 #include "kernels2.cuh"
+#include "reduce.cuh"
 
 using namespace cyr;
 
@@ -71,7 +72,7 @@ struct cyrsoxs_ctx {
     bool plan_dirty = true;
     unsigned long long null_pattern = ~0ull;
     // workspace
-    DevBuf A1, A2, A3, img, twx, twy, twz, stage_out[2];
+    DevBuf A1, A2, A3, img, twx, twy, twz, stage_out[2], red;
     // last run
     cyrsoxs_stats stats{};
     cudaStream_t last_stream = nullptr;
@@ -591,7 +592,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
     clear_prof(c);
     for (void *p : c->owned_morph) cudaFree(p);
     for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
-                      &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind})
+                      &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind, &c->red})
         release(*b);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     for (int i = 0; i < 2; ++i) {
@@ -948,6 +949,45 @@ cyrsoxs_status cyrsoxs_get_stats(cyrsoxs_ctx *c, cyrsoxs_stats *stats)
         }
     }
     *stats = c->stats;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_reduce(cyrsoxs_ctx *c, void *cuda_stream, const float *d_images, const unsigned int *d_counts,
+                              int n_energy, int n_bins, double sector_half_width_deg, float *d_I, float *d_A, float *d_isi)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (!d_images || !d_I) return fail(c, CYRSOXS_ERR_INVALID_ARG, "reduce: images or I output is NULL");
+    if (n_energy < 1 || n_bins < 1 || n_bins > 4096) return fail(c, CYRSOXS_ERR_INVALID_ARG, "reduce: n_energy >= 1 and 1 <= n_bins <= 4096");
+    if (!(sector_half_width_deg > 0.0) || !(sector_half_width_deg <= 45.0))
+        return fail(c, CYRSOXS_ERR_INVALID_ARG, "reduce: sector half width must be in (0, 45] degrees");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    const size_t nb = (size_t)n_energy * 3 * n_bins;
+    const size_t bytes = sizeof(double) * nb + sizeof(double) * n_energy + sizeof(unsigned int) * nb;
+    cyrsoxs_status s = ensure(c, c->red, bytes);
+    if (s != CYRSOXS_OK) return s;
+    CUDA_TRY(c, cudaMemsetAsync(c->red.p, 0, bytes, st));
+    ReduceParams p{};
+    p.Nx = c->Nx; p.Ny = c->Ny; p.n_bins = n_bins;
+    p.rho = (double)c->Nx / (double)c->Ny;
+    p.tan_w = tan(sector_half_width_deg * (kPi / 180.0));
+    p.img = d_images; p.cnt = d_counts;
+    p.acc = (double *)c->red.p; p.total = p.acc + nb; p.num = (unsigned int *)(p.total + n_energy);
+    // enough CTAs to fill the machine, at least 4 rows each so the shared-memory bins are amortised
+    const int want = std::max(1, 4 * c->n_sm / n_energy);
+    p.rows_per_cta = std::max(4, (c->Ny + want - 1) / want);
+    const dim3 grid((c->Ny + p.rows_per_cta - 1) / p.rows_per_cta, n_energy);
+    const size_t smem = (size_t)3 * n_bins * (sizeof(double) + sizeof(unsigned int));
+    static bool attr_done[64] = {false};
+    if (smem > 48 * 1024 && !attr_done[c->device & 63]) {
+        CUDA_TRY(c, cudaFuncSetAttribute(k_reduce_accumulate, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 4096 * 12));
+        attr_done[c->device & 63] = true;
+    }
+    k_reduce_accumulate<<<grid, 256, smem, st>>>(p);
+    CUDA_TRY(c, cudaGetLastError());
+    const int tot = n_energy * n_bins;
+    k_reduce_finalize<<<(tot + 255) / 256, 256, 0, st>>>(n_energy, n_bins, p.acc, p.num, p.total, c->dqx * c->dqy, d_I, d_A, d_isi);
+    CUDA_TRY(c, cudaGetLastError());
     return CYRSOXS_OK;
 }
 

@@ -199,3 +199,52 @@ def test_host_output_and_host_morphology():
     ctx.run(out.data_ptr(), s)
     torch.cuda.synchronize()
     compare(out.numpy(), None, ref, rcnt, "host-io")
+
+
+@pytest.mark.parametrize("shape,n_bins,width", [((64, 64, 1), 32, 20.0), ((128, 32, 4), 70, 10.0), ((32, 64, 2), 16, 45.0)])
+def test_reductions_match_oracle(shape, n_bins, width):
+    """cyrsoxs_reduce (NEXT-1: I(|q|), anisotropy, ISI) on the GPU path's own images against the
+    oracle's reductions of the oracle's images: bins are integer decisions (compared through the
+    means of a coordinate image, exactly), values within the image tolerance."""
+    import torch
+    import oracle
+    from paper_2209_13121_b200 import binding
+    nx, ny, nz = shape
+    w = W.tiny(seed=31 + nx, nx=nx, ny=ny, nz=nz, n_mat=3, n_energy=3, voxel_nm=2.5, ewald=W.EWALD_NEAREST)
+    ref, rcnt = oracle_run(w)
+    out, cnt, ctx = binding.simulate(w, want_counts=True)[:3]
+    I = torch.zeros((3, n_bins), device="cuda"); A = torch.zeros_like(I); isi = torch.zeros(3, device="cuda")
+    ctx.reduce(out.data_ptr(), cnt.data_ptr(), 3, n_bins, width, I.data_ptr(), A.data_ptr(), isi.data_ptr(),
+               torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    I, A, isi = I.cpu().numpy(), A.cpu().numpy(), isi.cpu().numpy()
+    for e in range(3):
+        rI, rA, rn, risi = oracle.reductions(ref[e], rcnt[e], w.voxel_nm, n_bins, width)
+        scale = rI.max()
+        assert np.abs(I[e] - rI).max() <= 2e-5 * scale, (e, np.abs(I[e] - rI).max() / scale)
+        sig = rI > 1e-4 * scale                         # A is a ratio: compare where the bin carries signal
+        assert np.abs(A[e] - rA)[sig].max() <= 1e-4, (e, np.abs(A[e] - rA)[sig].max())
+        assert abs(isi[e] - risi) <= 2e-5 * abs(risi)
+    # the binning itself, bit-exact: reduce an image whose value is its own pixel index
+    # (sums of distinct integers < 2^24 identify the set of pixels of every bin and sector)
+    idx = torch.arange(nx * ny, dtype=torch.float32, device="cuda").reshape(1, ny, nx).contiguous()
+    I1 = torch.zeros((1, n_bins), device="cuda"); A1 = torch.zeros_like(I1); s1 = torch.zeros(1, device="cuda")
+    ctx.reduce(idx.data_ptr(), None, 1, n_bins, width, I1.data_ptr(), A1.data_ptr(), s1.data_ptr(),
+               torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    rI, rA, rn, risi = oracle.reductions(idx[0].cpu().numpy().astype(np.float64), None, w.voxel_nm, n_bins, width)
+    assert np.allclose(I1[0].cpu().numpy(), rI, rtol=2e-7, atol=0)
+    assert np.allclose(A1[0].cpu().numpy(), rA, rtol=0, atol=2e-7)
+    assert np.isclose(float(s1[0]), risi, rtol=2e-7)
+
+
+def test_reduce_rejects_bad_arguments():
+    import torch
+    from paper_2209_13121_b200 import binding
+    ctx = binding.Context(16, 16, 1, 1, 2.0)
+    img = torch.zeros((1, 16, 16), device="cuda"); I = torch.zeros((1, 8), device="cuda")
+    for bins, width in [(0, 20.0), (5000, 20.0), (8, 0.0), (8, 60.0)]:
+        with pytest.raises(binding.CyrsoxsError) as ei:
+            ctx.reduce(img.data_ptr(), None, 1, bins, width, I.data_ptr())
+        assert ei.value.status == binding.ERR_INVALID_ARG
+    ctx.close()
