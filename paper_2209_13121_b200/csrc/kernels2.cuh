@@ -80,6 +80,10 @@ k_col2(const ColParams p)
 // butterfly there, and the remaining stages through a 4-pack shared-memory buffer per row; the
 // last stage stores the window [lo, lo + W) of bins straight to out[pack][row][slot].
 constexpr int XB2_PB = 4;       // packs buffered per row between flushes
+static_assert(XB2_PB >= 4, "an aligned material emits up to 4 packs between flush checks");
+// CTAs per SM the register allocation aims at: 3 (80 registers, a few spilled values) measured 9-12 % faster
+// than 2 (126 registers) on CFG2, CFG3 and CFG5 -- the kernel is latency bound at 16 warps per SM.
+constexpr int XB2_MINB = 3;
 
 template <int LOGN> struct XB2Cfg {
     static constexpr int N = 1 << LOGN;
@@ -91,7 +95,7 @@ template <int LOGN> struct XB2Cfg {
 };
 
 template <int LOGN>
-__global__ void __launch_bounds__(XB2Cfg<LOGN>::THREADS, 2)
+__global__ void __launch_bounds__(XB2Cfg<LOGN>::THREADS, XB2_MINB)
 k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, Window wx, int pitch,
           const float2 *__restrict__ tw)
 {
@@ -126,10 +130,12 @@ k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
                 if (row_ok) o[sl] = make_float2(0.f, 0.f);
         }
     };
-    auto emit = [&](const float (&a)[R0], const float (&b)[R0]) {
+    // one complex pack from two real fields given as generators fa(s), fb(s) of the thread's voxel s:
+    // the products are formed here, right before the stage-0 butterfly, so only w, d and phi stay live
+    auto emit = [&](auto fa, auto fb) {
         float2 v[R0];
 #pragma unroll
-        for (int s = 0; s < R0; ++s) v[s] = make_float2(a[s], b[s]);
+        for (int s = 0; s < R0; ++s) v[s] = make_float2(fa(s), fb(s));
         F::stage0(v);
         if constexpr (NST > 1) { F::stage0_store(Lrow + nbuf * N, li, v); ++nbuf; }
         else { store_global(pack_out, v); ++pack_out; }
@@ -181,28 +187,33 @@ k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
                 th[s] = __ldg(mp.theta[m] + vox0 + (size_t)s * T);
                 ps[s] = __ldg(mp.psi[m] + vox0 + (size_t)s * T);
             }
-            float fw[R0], fxx[R0], fyy[R0], fxy[R0], fxz[R0], fyz[R0];
+            float w[R0], dx[R0], dy[R0], dz[R0];
 #pragma unroll
             for (int s = 0; s < R0; ++s) {
-                const float w = ph[s] * S_[s];
+                w[s] = ph[s] * S_[s];
                 float st, ct, sp, cp;
                 sincosf(th[s], &st, &ct);
                 sincosf(ps[s], &sp, &cp);
-                const float dx = cp * st, dy = sp * st, dz = ct;
-                const float wdx = w * dx, wdy = w * dy;
-                fw[s] = w; fxx[s] = wdx * dx; fyy[s] = wdy * dy; fxy[s] = wdx * dy; fxz[s] = wdx * dz; fyz[s] = wdy * dz;
+                dx[s] = cp * st; dy[s] = sp * st; dz[s] = ct;
             }
+            auto f_ph = [&](int s) { return ph[s]; };
+            auto f_w = [&](int s) { return w[s]; };
+            auto f_xx = [&](int s) { return (w[s] * dx[s]) * dx[s]; };
+            auto f_yy = [&](int s) { return (w[s] * dy[s]) * dy[s]; };
+            auto f_xy = [&](int s) { return (w[s] * dx[s]) * dy[s]; };
+            auto f_xz = [&](int s) { return (w[s] * dx[s]) * dz[s]; };
+            auto f_yz = [&](int s) { return (w[s] * dy[s]) * dz[s]; };
             if (has_carry) {
-                emit(carry, ph); emit(fw, fxx); emit(fyy, fxy); emit(fxz, fyz);
+                emit([&](int s) { return carry[s]; }, f_ph); emit(f_w, f_xx); emit(f_yy, f_xy); emit(f_xz, f_yz);
                 has_carry = false;
             } else {
-                emit(ph, fw); emit(fxx, fyy); emit(fxy, fxz);
+                emit(f_ph, f_w); emit(f_xx, f_yy); emit(f_xy, f_xz);
 #pragma unroll
-                for (int s = 0; s < R0; ++s) carry[s] = fyz[s];
+                for (int s = 0; s < R0; ++s) carry[s] = f_yz(s);
                 has_carry = true;
             }
         } else {
-            if (has_carry) { emit(carry, ph); has_carry = false; }
+            if (has_carry) { emit([&](int s) { return carry[s]; }, [&](int s) { return ph[s]; }); has_carry = false; }
             else {
 #pragma unroll
                 for (int s = 0; s < R0; ++s) carry[s] = ph[s];
@@ -212,10 +223,7 @@ k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
     }
     if (has_carry) {
         if (nbuf + 1 > XB2_PB) flush();
-        float zero[R0];
-#pragma unroll
-        for (int s = 0; s < R0; ++s) zero[s] = 0.f;
-        emit(carry, zero);
+        emit([&](int s) { return carry[s]; }, [](int) { return 0.f; });
     }
     flush();
 }
