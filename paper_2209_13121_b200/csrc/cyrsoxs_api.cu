@@ -52,8 +52,9 @@ struct cyrsoxs_ctx {
     // angles
     int nA = 0;
     std::vector<double2> cs;
-    DevBuf d_cs, d_csf, d_tiles[4];            // rotate tile tables for EG = 1, 2, 4, 8
-    int n_tiles[4] = {0, 0, 0, 0};
+    DevBuf d_tiles[8];                          // rotate tile tables for EG = 1, 2, 4, 8 and AS = 1, 4
+    DevBuf d_cs, d_csf;
+    int n_tiles[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     int eg = 1;                                 // energies interleaved per image group in this run
     unsigned long long plan_key = 0;            // what the cached energy batch was planned for
     size_t plan_fixed = 0, plan_per_e = 0;
@@ -164,13 +165,20 @@ Window make_window(int N, int K, bool symmetric)
 
 int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
-// Output tiles of the rotate kernel for image layout EG = 1 << lg, nearest to q = 0 first
-// (see k_rotate_avg); built on first use.
-cyrsoxs_status make_rotate_tiles(cyrsoxs_ctx *c, int lg)
+// Output tiles of the rotate kernel for image layout EG = 1 << lg and AS angle slices (slot
+// lg + 4 (AS == 4)), nearest to q = 0 first (see k_rotate_avg); built on first use.
+template <int AS> void rot_tile_dims(int lg, int &TW, int &TH)
 {
-    if (c->n_tiles[lg]) return CYRSOXS_OK;
-    const int TW = lg == 0 ? RotMap<1>::TW : lg == 1 ? RotMap<2>::TW : lg == 2 ? RotMap<4>::TW : RotMap<8>::TW;
-    const int TH = lg == 0 ? RotMap<1>::TH : lg == 1 ? RotMap<2>::TH : lg == 2 ? RotMap<4>::TH : RotMap<8>::TH;
+    TW = lg == 0 ? RotMap<1, AS>::TW : lg == 1 ? RotMap<2, AS>::TW : lg == 2 ? RotMap<4, AS>::TW : RotMap<8, AS>::TW;
+    TH = lg == 0 ? RotMap<1, AS>::TH : lg == 1 ? RotMap<2, AS>::TH : lg == 2 ? RotMap<4, AS>::TH : RotMap<8, AS>::TH;
+}
+
+cyrsoxs_status make_rotate_tiles(cyrsoxs_ctx *c, int lg, int as)
+{
+    const int slot = lg + (as == 4 ? 4 : 0);
+    if (c->n_tiles[slot]) return CYRSOXS_OK;
+    int TW, TH;
+    if (as == 4) rot_tile_dims<4>(lg, TW, TH); else rot_tile_dims<1>(lg, TW, TH);
     const int ntx = (c->Nx + TW - 1) / TW, nty = (c->Ny + TH - 1) / TH;
     const double rho = (double)c->Nx / (double)c->Ny;
     std::vector<std::pair<double, uint32_t>> t;
@@ -183,10 +191,10 @@ cyrsoxs_status make_rotate_tiles(cyrsoxs_ctx *c, int lg)
     std::sort(t.begin(), t.end());
     std::vector<uint32_t> h(t.size());
     for (size_t i = 0; i < t.size(); ++i) h[i] = t[i].second;
-    cyrsoxs_status st = ensure(c, c->d_tiles[lg], sizeof(uint32_t) * h.size());
+    cyrsoxs_status st = ensure(c, c->d_tiles[slot], sizeof(uint32_t) * h.size());
     if (st != CYRSOXS_OK) return st;
-    CUDA_TRY(c, cudaMemcpy(c->d_tiles[lg].p, h.data(), sizeof(uint32_t) * h.size(), cudaMemcpyHostToDevice));
-    c->n_tiles[lg] = (int)h.size();
+    CUDA_TRY(c, cudaMemcpy(c->d_tiles[slot].p, h.data(), sizeof(uint32_t) * h.size(), cudaMemcpyHostToDevice));
+    c->n_tiles[slot] = (int)h.size();
     return CYRSOXS_OK;
 }
 
@@ -308,23 +316,36 @@ template <int EG> dim3 ewald_grid(const cyrsoxs_ctx *c, int eb)
 template <int EG>
 cyrsoxs_status launch_rotate_t(cyrsoxs_ctx *c, cudaStream_t st, RotateParams p, int eb, int lg)
 {
-    cyrsoxs_status s = make_rotate_tiles(c, lg);
-    if (s != CYRSOXS_OK) return s;
-    p.tiles = (const uint32_t *)c->d_tiles[lg].p;
-    const long long tiles = c->n_tiles[lg];
-    const int ng = (eb + EG - 1) / EG;
+    static const int force_ua = getenv("CYRSOXS_ROT_UA") ? atoi(getenv("CYRSOXS_ROT_UA")) : 0;      // tuning aids
+    static const int force_as = getenv("CYRSOXS_ROT_AS") ? atoi(getenv("CYRSOXS_ROT_AS")) : 0;
     // groups per CTA: all of them (up to ROT_GMAX), so the cells of an angle are computed once per pixel
-    static const int force_ua = getenv("CYRSOXS_ROT_UA") ? atoi(getenv("CYRSOXS_ROT_UA")) : 0;      // tuning aid
+    const int ng = (eb + EG - 1) / EG;
     const int gpc = std::min(ng, ROT_GMAX);
+    const int slices_y = (ng + gpc - 1) / gpc;
     p.gpc = gpc;
-    const dim3 grid((unsigned)tiles, (ng + gpc - 1) / gpc);
+    // angle slices: 4 threads per pixel when one per pixel leaves the machine under-filled and there are
+    // several energy groups to walk through per angle (cfg2: 38 -> 35 us; no gain on cfg1's single energy)
+    const long long px_ctas = ((long long)c->Nx * c->Ny * EG + 255) / 256 * slices_y;
+    int as = (px_ctas < 4LL * c->n_sm && c->nA >= 8 && ng >= 2) ? 4 : 1;
+    if (force_as == 1 || force_as == 4) as = force_as;
+    cyrsoxs_status s = make_rotate_tiles(c, lg, as);
+    if (s != CYRSOXS_OK) return s;
+    const int slot = lg + (as == 4 ? 4 : 0);
+    p.tiles = (const uint32_t *)c->d_tiles[slot].p;
+    const dim3 grid((unsigned)c->n_tiles[slot], slices_y);
     const size_t smem = (size_t)gpc * 256 * 8;
     // angles in flight: 1 when the grid fills the machine several times over (occupancy hides the
-    // load latency; measured best on cfg4), 4 when it does not (cfg1, cfg2)
-    const int ua = force_ua ? force_ua : ((long long)grid.x * grid.y >= 16LL * c->n_sm ? 1 : 4);
-    if (ua == 4) k_rotate_avg<EG, 4, 2><<<grid, 256, smem, st>>>(p);
-    else if (ua == 2) k_rotate_avg<EG, 2, 3><<<grid, 256, smem, st>>>(p);
-    else k_rotate_avg<EG, 1, 4><<<grid, 256, smem, st>>>(p);
+    // load latency; measured best on cfg4), more when it does not
+    const int ua = force_ua ? force_ua : ((long long)grid.x * grid.y >= 16LL * c->n_sm ? 1 : (as == 4 ? 2 : 4));
+    if (as == 4) {
+        if (ua == 4) k_rotate_avg<EG, 4, 2, 4><<<grid, 256, smem, st>>>(p);
+        else if (ua == 2) k_rotate_avg<EG, 2, 3, 4><<<grid, 256, smem, st>>>(p);
+        else k_rotate_avg<EG, 1, 4, 4><<<grid, 256, smem, st>>>(p);
+    } else {
+        if (ua == 4) k_rotate_avg<EG, 4, 2, 1><<<grid, 256, smem, st>>>(p);
+        else if (ua == 2) k_rotate_avg<EG, 2, 3, 1><<<grid, 256, smem, st>>>(p);
+        else k_rotate_avg<EG, 1, 4, 1><<<grid, 256, smem, st>>>(p);
+    }
     CUDA_TRY(c, cudaGetLastError());
     return CYRSOXS_OK;
 }
@@ -591,7 +612,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
     if (!c) return;
     clear_prof(c);
     for (void *p : c->owned_morph) cudaFree(p);
-    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
+    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->d_tiles[4], &c->d_tiles[5], &c->d_tiles[6], &c->d_tiles[7], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
                       &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind, &c->red})
         release(*b);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);

@@ -564,12 +564,19 @@ struct RotateParams {
     int gpc;                    // energy groups per CTA (blockIdx.y slices the groups)
 };
 
-// 256 threads: 8 warps as 4 (x) by 2 (y); a warp covers WPW x WPH pixels times EG energies.
-template <int EG> struct RotMap {
+// 256 threads = AS angle slices x WS = 8 / AS warps; the WS warps of a slice tile WSX x WSY warp
+// patches, a warp covers WPW x WPH pixels times EG energies.  AS > 1 (small images: too few
+// tiles to fill the machine, and every thread a long serial chain over the angles) gives every
+// pixel AS threads that each take a contiguous share of the angles; their partial sums are added
+// in slice order at the end, so the result does not depend on scheduling.
+template <int EG, int AS> struct RotMap {
     static constexpr int WP = 32 / EG;                                        // pixels per warp
     static constexpr int WPW = WP >= 16 ? 8 : (WP == 8 ? 4 : 2);              // 8x4, 8x2, 4x2, 2x2
     static constexpr int WPH = WP / WPW;
-    static constexpr int TW = 4 * WPW, TH = 2 * WPH;                          // CTA tile
+    static constexpr int WS = 8 / AS;                                         // warps per slice
+    static constexpr int WSX = WS >= 4 ? (WS == 8 ? 4 : 2) : WS;              // 4x2, 2x2, 2x1, 1x1
+    static constexpr int WSY = WS / WSX;
+    static constexpr int TW = WSX * WPW, TH = WSY * WPH;                      // CTA tile
 };
 
 // reach2[e] = (k_e/dq_x + 3)^2: an output pixel whose distance from q = 0 (measured in x
@@ -583,11 +590,11 @@ template <int EG> struct RotMap {
 // whose running sums and counts live in shared memory between chunks.
 constexpr int ROT_GMAX = 16;      // most energy groups per CTA (RotateParams::gpc <= ROT_GMAX)
 
-template <int EG, int UA, int MINB>
+template <int EG, int UA, int MINB, int AS>
 __global__ void __launch_bounds__(256, MINB)
 k_rotate_avg(const RotateParams p)
 {
-    using M = RotMap<EG>;
+    using M = RotMap<EG, AS>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n_groups = (p.n_energy + EG - 1) / EG;
     const int g0 = blockIdx.y * p.gpc;
@@ -597,9 +604,11 @@ k_rotate_avg(const RotateParams p)
     const uint32_t tile = __ldg(p.tiles + blockIdx.x);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int sub = lane % EG, lp = lane / EG;
-    const int ix = (int)(tile & 0xffffu) * M::TW + (warp & 3) * M::WPW + lp % M::WPW;
-    const int iy = (int)(tile >> 16) * M::TH + (warp >> 2) * M::WPH + lp / M::WPW;
-    if (ix >= p.Nx || iy >= p.Ny) return;                       // no block-wide barrier below
+    const int slice = warp / M::WS, wl = warp % M::WS;
+    const int ix = (int)(tile & 0xffffu) * M::TW + (wl % M::WSX) * M::WPW + lp % M::WPW;
+    const int iy = (int)(tile >> 16) * M::TH + (wl / M::WSX) * M::WPH + lp / M::WPW;
+    const bool inside = ix < p.Nx && iy < p.Ny;
+    if (AS == 1 && !inside) return;                             // AS == 1: no block-wide barrier below
     const size_t plane = (size_t)p.Ny * p.Nx * EG;               // float4 per energy group
     const float4 *img = p.img + (size_t)g0 * plane + sub;
     const double rho = p.rho;
@@ -612,13 +621,16 @@ k_rotate_avg(const RotateParams p)
     unsigned int live = 0;
     for (int j = 0; j < ng; ++j) {
         const int e = (g0 + j) * EG + sub;
-        if (e < p.n_energy && r2 <= __ldg(p.reach2 + e)) live |= 1u << j;
+        if (inside && e < p.n_energy && r2 <= __ldg(p.reach2 + e)) live |= 1u << j;
         s_sum[j * 256 + tid] = 0.f;
         s_cnt[j * 256 + tid] = 0u;
     }
-    const int na = live ? p.n_angles : 0;
+    // this slice's share of the angles: [a_begin, na)
+    const int per = (p.n_angles + AS - 1) / AS;
+    const int a_begin = slice * per;
+    const int na = live ? min(p.n_angles, a_begin + per) : 0;
     const int rowq = p.Nx * EG;
-    for (int a0 = 0; a0 < na; a0 += UA) {
+    for (int a0 = a_begin; a0 < na; a0 += UA) {
         int o00[UA], ox[UA], oy[UA];
         float w00[UA], w10[UA], w01[UA], w11[UA], wx[UA], wy[UA], wz[UA];
         bool ok[UA];
@@ -666,12 +678,20 @@ k_rotate_avg(const RotateParams p)
             s_cnt[j * 256 + tid] = cnt;
         }
     }
+    if (AS > 1) __syncthreads();
+    if (slice != 0 || !inside) return;
     for (int j = 0; j < ng; ++j) {
         const int e = (g0 + j) * EG + sub;
         if (e < p.n_energy) {
             const size_t o = ((size_t)e * p.Ny + iy) * p.Nx + ix;
-            const unsigned int cnt = s_cnt[j * 256 + tid];
-            p.out[o] = cnt ? s_sum[j * 256 + tid] / (float)cnt : 0.f;
+            float sum = s_sum[j * 256 + tid];
+            unsigned int cnt = s_cnt[j * 256 + tid];
+#pragma unroll
+            for (int sl = 1; sl < AS; ++sl) {
+                sum += s_sum[j * 256 + tid + sl * M::WS * 32];
+                cnt += s_cnt[j * 256 + tid + sl * M::WS * 32];
+            }
+            p.out[o] = cnt ? sum / (float)cnt : 0.f;
             if (p.counts) p.counts[o] = cnt;
         }
     }
