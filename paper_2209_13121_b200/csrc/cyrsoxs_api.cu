@@ -266,9 +266,37 @@ template <int LOGN> cyrsoxs_status launch_colpass_t(cyrsoxs_ctx *c, cudaStream_t
     return CYRSOXS_OK;
 }
 
+template <int LOGN, int PW> cyrsoxs_status launch_colpass_pair_t(cyrsoxs_ctx *c, cudaStream_t st, ColParams p, int n_lo, int n_hi, int pitch)
+{
+    using Cfg = Col2PCfg<LOGN, PW>;
+    static bool attr_done[64] = {false};
+    if (!attr_done[c->device & 63]) {
+        CUDA_TRY(c, cudaFuncSetAttribute(k_col2p<LOGN, PW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        attr_done[c->device & 63] = true;
+    }
+    p.n_tiles = pitch / Cfg::TX;
+    dim3 grid((unsigned)(p.n_tiles * n_lo), (unsigned)n_hi);
+    k_col2p<LOGN, PW><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    CUDA_TRY(c, cudaGetLastError());
+    return CYRSOXS_OK;
+}
+
 cyrsoxs_status launch_colpass(cyrsoxs_ctx *c, cudaStream_t st, int N, const ColParams &p, int n_lo, int n_hi, int pitch)
 {
-    switch (ilog2(N)) {
+    // lengths 128 .. 1024 take the two-columns-per-thread kernel (measured faster at every one of them:
+    // cfg2 z 29 -> 25 us, cfg3 z 0.75 -> 0.65 / y 0.49 -> 0.40 ms, cfg5 z 7.4 -> 4.5 / y 4.1 -> 3.1 ms)
+    static const int pair_min = getenv("CYRSOXS_PAIR_MIN") ? atoi(getenv("CYRSOXS_PAIR_MIN")) : 7;      // tuning aid
+    const int lg = ilog2(N);
+    // all strides are multiples of 2 elements (pitch is a multiple of 32), so 128-bit accesses are aligned
+    if (lg >= pair_min) {
+        switch (lg) {
+        case 7: return launch_colpass_pair_t<7, 8>(c, st, p, n_lo, n_hi, pitch);
+        case 8: return launch_colpass_pair_t<8, 8>(c, st, p, n_lo, n_hi, pitch);
+        case 9: return launch_colpass_pair_t<9, 8>(c, st, p, n_lo, n_hi, pitch);
+        case 10: return launch_colpass_pair_t<10, 8>(c, st, p, n_lo, n_hi, pitch);
+        }
+    }
+    switch (lg) {
 #define CASE(L) case L: return launch_colpass_t<L>(c, st, p, n_lo, n_hi, pitch);
         CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11)
 #undef CASE

@@ -58,6 +58,12 @@ template <int TX> struct ColMap {
     }
 };
 
+// Pairs of lines as float4: PW pairs side by side, element i of pair c at (i PW + c).  With PW = 8 a
+// quarter-warp (one 128-bit wavefront) covers one full 128-byte row, so no swizzle is needed.
+template <int PW> struct PairMap {
+    __device__ __forceinline__ static int at(int i) { return i * PW; }
+};
+
 template <int LOGN, class Map> struct RegFft {
     using S = RSched<LOGN>;
     static constexpr int N = 1 << LOGN;
@@ -123,6 +129,47 @@ template <int LOGN, class Map> struct RegFft {
             const int o = (j / NS) * (NS * R) + (j & (NS - 1));
 #pragma unroll
             for (int t = 0; t < R; ++t) L[Map::at(o + t * NS)] = v[b * R + t];
+        }
+    }
+
+    // ---- two adjacent lines at once, kept in shared memory as float4 (line a in .xy, line b in .zw) ----
+    __device__ __forceinline__ static void stage0_store2(float4 *L, int li, const float2 (&va)[R0], const float2 (&vb)[R0])
+    {
+#pragma unroll
+        for (int t = 0; t < R0; ++t) L[Map::at(li * R0 + t)] = make_float4(va[t].x, va[t].y, vb[t].x, vb[t].y);
+    }
+
+    template <int ST>
+    __device__ __forceinline__ static void stage_load2(const float4 *L, int li, const float2 (&w)[R0], float2 (&va)[R0],
+                                                       float2 (&vb)[R0])
+    {
+        constexpr int R = S::R[ST], B = R0 / R;
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int j = li + b * T;
+#pragma unroll
+            for (int s = 0; s < R; ++s) {
+                const float4 q = L[Map::at(j + s * (N / R))];
+                va[b * R + s] = make_float2(q.x, q.y); vb[b * R + s] = make_float2(q.z, q.w);
+            }
+#pragma unroll
+            for (int s = 1; s < R; ++s) { va[b * R + s] = cmul(va[b * R + s], w[b * R + s]); vb[b * R + s] = cmul(vb[b * R + s], w[b * R + s]); }
+            Dft<R>::run(&va[b * R]);
+            Dft<R>::run(&vb[b * R]);
+        }
+    }
+
+    template <int ST>
+    __device__ __forceinline__ static void stage_store2(float4 *L, int li, const float2 (&va)[R0], const float2 (&vb)[R0])
+    {
+        constexpr int R = S::R[ST], B = R0 / R, NS = ns_of(ST);
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int j = li + b * T;
+            const int o = (j / NS) * (NS * R) + (j & (NS - 1));
+#pragma unroll
+            for (int t = 0; t < R; ++t)
+                L[Map::at(o + t * NS)] = make_float4(va[b * R + t].x, va[b * R + t].y, vb[b * R + t].x, vb[b * R + t].y);
         }
     }
 

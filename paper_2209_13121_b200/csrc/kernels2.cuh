@@ -70,6 +70,73 @@ k_col2(const ColParams p)
     }
 }
 
+// Same pass with two adjacent columns per thread (128-bit global loads and stores, float4 in shared
+// memory): a tile is 16 columns = 128-byte row segments at half the threads of k_col2's 16-column
+// configuration.  Used where k_col2 would otherwise fall back to 8-column tiles (N = 512).
+template <int LOGN, int PW_> struct Col2PCfg {
+    static constexpr int N = 1 << LOGN;
+    static constexpr int PW = PW_, TX = 2 * PW;
+    using F = RegFft<LOGN, PairMap<PW>>;
+    static constexpr int T = F::T;
+    static constexpr int THREADS = T * PW;
+    static constexpr size_t SMEM = sizeof(float4) * (size_t)N * PW;
+};
+
+template <int LOGN, int PW_>
+__global__ void __launch_bounds__(Col2PCfg<LOGN, PW_>::THREADS)
+k_col2p(const ColParams p)
+{
+    using Cfg = Col2PCfg<LOGN, PW_>;
+    using F = typename Cfg::F;
+    constexpr int N = Cfg::N, TX = Cfg::TX, PW = Cfg::PW, T = Cfg::T, R0 = F::R0, NST = F::NST;
+    static_assert(NST > 1, "pair pass is for long transforms");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float4 *sm = reinterpret_cast<float4 *>(smem_raw);
+    const int tid = threadIdx.x;
+    const int c = tid % PW, li = tid / PW;
+    const int tile = blockIdx.x % p.n_tiles, lo = blockIdx.x / p.n_tiles, hi = blockIdx.y;
+
+    const float2 *src = p.in + (size_t)hi * p.in_hi + (size_t)lo * p.in_lo + (size_t)tile * TX + 2 * c;
+    float2 va[R0], vb[R0];
+#pragma unroll
+    for (int s = 0; s < R0; ++s) {
+        const float4 q = __ldcs(reinterpret_cast<const float4 *>(src + (size_t)(li + s * T) * p.in_row));
+        va[s] = make_float2(q.x, q.y); vb[s] = make_float2(q.z, q.w);
+    }
+    F::stage0(va);
+    F::stage0(vb);
+    float4 *L = sm + c;
+    F::stage0_store2(L, li, va, vb);
+    float2 w[R0];
+    if constexpr (NST > 2) {
+        __syncthreads();
+        F::template load_tw<1>(p.tw, li, w);
+        F::template stage_load2<1>(L, li, w, va, vb);
+        __syncthreads();
+        F::template stage_store2<1>(L, li, va, vb);
+    }
+    if constexpr (NST > 3) {
+        __syncthreads();
+        F::template load_tw<2>(p.tw, li, w);
+        F::template stage_load2<2>(L, li, w, va, vb);
+        __syncthreads();
+        F::template stage_store2<2>(L, li, va, vb);
+    }
+    __syncthreads();
+    F::template load_tw<NST - 1>(p.tw, li, w);
+    F::template stage_load2<NST - 1>(L, li, w, va, vb);
+    float2 *dst = p.out + (size_t)hi * p.out_hi + (size_t)lo * p.out_lo + (size_t)tile * TX + 2 * c;
+#pragma unroll
+    for (int m = 0; m < R0; ++m) {
+        const int k = li + T * m;
+        const int sl = (k - p.win.lo) & (N - 1);
+        if (sl < p.win.W) {
+            const float2 a = va[F::out_reg(m)], b = vb[F::out_reg(m)];
+            *reinterpret_cast<float4 *>(dst + (size_t)sl * p.out_row) = make_float4(a.x, a.y, b.x, b.y);
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // x pass of SPECTRAL_BASIS (DESIGN 7.2).  The energy-independent real fields, in material order
 //   aligned material:   phi, w = phi S, w dx dx, w dy dy, w dx dy, w dx dz, w dy dz      (7)

@@ -24,7 +24,7 @@ def _gpu(w, alg, images=False):
 
 @pytest.mark.parametrize("alg", ALGS)
 @pytest.mark.parametrize("mode", [W.EWALD_NEAREST, W.EWALD_TRILINEAR])
-@pytest.mark.parametrize("shape", [(8, 8, 4), (32, 16, 8), (16, 64, 2), (64, 32, 1), (4, 4, 16)])
+@pytest.mark.parametrize("shape", [(8, 8, 4), (32, 16, 8), (16, 64, 2), (64, 32, 1), (4, 4, 16), (16, 512, 2), (8, 4, 512), (1024, 4, 1), (8, 128, 256), (4, 1024, 2)])
 def test_tiny_random(shape, mode, alg):
     nx, ny, nz = shape
     w = W.tiny(seed=100 + nx + nz, nx=nx, ny=ny, nz=nz, n_mat=3, n_energy=3, voxel_nm=2.0, ewald=mode)
