@@ -890,9 +890,11 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
 
     cyrsoxs_status s;
     if (c->plan_dirty && (s = build_basis_plan(c)) != CYRSOXS_OK) return s;
-    // AUTO: the basis needs n_pack complex transforms per run, PER_ENERGY 5 per energy
+    // AUTO: the basis needs n_pack complex transforms per run, PER_ENERGY 5 per energy; a basis transform
+    // (register-first x pass, real fields) costs about half of a PER_ENERGY one (measured on cfg3: 0.31 ms
+    // per pack against 0.6 ms per field), hence the factor 2
     int alg = c->alg;
-    if (alg == CYRSOXS_ALG_AUTO) alg = (NCHI * c->nE > c->n_pack) ? CYRSOXS_ALG_SPECTRAL_BASIS : CYRSOXS_ALG_PER_ENERGY;
+    if (alg == CYRSOXS_ALG_AUTO) alg = (2 * NCHI * c->nE >= c->n_pack) ? CYRSOXS_ALG_SPECTRAL_BASIS : CYRSOXS_ALG_PER_ENERGY;
     const bool spectral = alg == CYRSOXS_ALG_SPECTRAL_BASIS;
 
     // plan: windows for the largest k, energy batch from the free memory
