@@ -110,6 +110,15 @@ cyrsoxs_status cyrsoxs_set_morphology_host(cyrsoxs_ctx *ctx, const float *const 
                                            const float *const *h_S, const float *const *h_theta,
                                            const float *const *h_psi, void *cuda_stream);
 
+/* Same, from the paper's own layout (Fig. 3): one DEVICE array of n_mat * Nx*Ny*Nz
+ * Real4 = float4 entries, voxels first and materials second (entry m*N + i), each entry
+ * (v_frac, s, Euler-phi, theta) = (phi, S, psi, theta) in this header's names.  The array is
+ * de-interleaved on `cuda_stream` into structure-of-arrays buffers owned by the context (the
+ * kernels read those; d_real4 is not referenced after the stream passes this call).  A material
+ * whose S is 0 in every voxel is detected and treated as isotropic.  16-byte alignment required.
+ * This call synchronises `cuda_stream` once (to read back the per-material max |S|). */
+cyrsoxs_status cyrsoxs_set_morphology_aos(cyrsoxs_ctx *ctx, const float *d_real4, void *cuda_stream);
+
 /* Energy list and the material library: HOST arrays, copied.  energies_eV has
  * n_energy entries (> 0); the four tables are [n_energy][n_mat] float32 with
  * n_par = 1 - delta_par + i beta_par, n_perp likewise.  The complex coefficients

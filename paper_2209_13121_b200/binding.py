@@ -19,7 +19,7 @@ STAGES = ("xpass", "zpass", "ypass", "ewald", "rotate")
 N_STAGES = len(STAGES)
 
 EXPORTS = [
-    "cyrsoxs_create", "cyrsoxs_set_morphology", "cyrsoxs_set_morphology_host",
+    "cyrsoxs_create", "cyrsoxs_set_morphology", "cyrsoxs_set_morphology_host", "cyrsoxs_set_morphology_aos",
     "cyrsoxs_set_optical_constants", "cyrsoxs_set_angles", "cyrsoxs_set_ewald", "cyrsoxs_set_algorithm",
     "cyrsoxs_set_counts_output", "cyrsoxs_set_profiling", "cyrsoxs_run", "cyrsoxs_num_angles",
     "cyrsoxs_get_stats", "cyrsoxs_reduce", "cyrsoxs_debug_fetch_images", "cyrsoxs_last_error", "cyrsoxs_destroy",
@@ -58,6 +58,7 @@ def load() -> C.CDLL:
     lib.cyrsoxs_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.POINTER(vp)]
     lib.cyrsoxs_set_morphology.argtypes = [vp, fpp, fpp, fpp, fpp]
     lib.cyrsoxs_set_morphology_host.argtypes = [vp, fpp, fpp, fpp, fpp, vp]
+    lib.cyrsoxs_set_morphology_aos.argtypes = [vp, vp, vp]
     lib.cyrsoxs_set_optical_constants.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp]
     lib.cyrsoxs_set_angles.argtypes = [vp, C.c_double, C.c_double, C.c_double]
     lib.cyrsoxs_set_ewald.argtypes = [vp, C.c_int]
@@ -151,6 +152,11 @@ class Context:
             tabs.append(_table(col))
         self._check(self.lib.cyrsoxs_set_morphology_host(self.h, *tabs, C.c_void_p(stream)))
         self._keep = keep
+
+    def set_morphology_aos(self, real4_ptr: int, stream: int = 0):
+        """The paper's Real4 layout: [n_mat][Nz*Ny*Nx] entries (phi, S, psi, theta), device memory."""
+        self._mats = None
+        self._check(self.lib.cyrsoxs_set_morphology_aos(self.h, real4_ptr, stream or None))
 
     def set_optical_constants(self, energies, delta_par, beta_par, delta_perp, beta_perp):
         import numpy as np

@@ -745,6 +745,57 @@ cyrsoxs_status cyrsoxs_set_morphology_host(cyrsoxs_ctx *c, const float *const *h
     return CYRSOXS_OK;
 }
 
+cyrsoxs_status cyrsoxs_set_morphology_aos(cyrsoxs_ctx *c, const float *d_real4, void *cuda_stream)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (!d_real4) return fail(c, CYRSOXS_ERR_INVALID_ARG, "morphology array is NULL");
+    if ((uintptr_t)d_real4 & 15) return fail(c, CYRSOXS_ERR_INVALID_ARG, "morphology array not 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    const size_t n = (size_t)c->Nx * c->Ny * c->Nz, bytes = sizeof(float) * n;
+    const size_t need = 4 * (size_t)c->n_mat;
+    if (c->owned_morph.size() != need) {
+        for (void *p : c->owned_morph) cudaFree(p);
+        c->owned_morph.clear();
+        for (size_t i = 0; i < need; ++i) {
+            void *d = nullptr;
+            cudaError_t e = cudaMalloc(&d, bytes);
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                for (void *p : c->owned_morph) cudaFree(p);
+                c->owned_morph.clear();
+                c->have_morph = false;
+                return fail(c, CYRSOXS_ERR_OOM, "cudaMalloc(morphology, %zu bytes): %s", bytes, cudaGetErrorString(e));
+            }
+            c->owned_morph.push_back(d);
+        }
+    }
+    cyrsoxs_status s = ensure(c, c->red, sizeof(unsigned int) * MAX_MAT);
+    if (s != CYRSOXS_OK) return s;
+    CUDA_TRY(c, cudaMemsetAsync(c->red.p, 0, sizeof(unsigned int) * MAX_MAT, st));
+    const int grid = std::min<long long>(((long long)n + 255) / 256, 8LL * c->n_sm);
+    for (int m = 0; m < c->n_mat; ++m) {
+        float *a[4];
+        for (int j = 0; j < 4; ++j) a[j] = (float *)c->owned_morph[4 * m + j];
+        k_aos_to_soa<<<grid, 256, 0, st>>>((const float4 *)d_real4 + (size_t)m * n, a[0], a[1], a[2], a[3], n,
+                                           (unsigned int *)c->red.p + m);
+        CUDA_TRY(c, cudaGetLastError());
+    }
+    unsigned int bits[MAX_MAT];
+    CUDA_TRY(c, cudaMemcpyAsync(bits, c->red.p, sizeof(unsigned int) * c->n_mat, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    for (int m = 0; m < c->n_mat; ++m) {
+        const bool aligned = bits[m] != 0;
+        c->mp.phi[m] = (const float *)c->owned_morph[4 * m];
+        c->mp.S[m] = aligned ? (const float *)c->owned_morph[4 * m + 1] : nullptr;
+        c->mp.theta[m] = aligned ? (const float *)c->owned_morph[4 * m + 2] : nullptr;
+        c->mp.psi[m] = aligned ? (const float *)c->owned_morph[4 * m + 3] : nullptr;
+    }
+    note_null_pattern(c);
+    c->have_morph = true;
+    return CYRSOXS_OK;
+}
+
 cyrsoxs_status cyrsoxs_set_optical_constants(cyrsoxs_ctx *c, int n_energy, const double *energies_eV,
                                              const float *delta_par, const float *beta_par,
                                              const float *delta_perp, const float *beta_perp)

@@ -86,4 +86,21 @@ __global__ void k_reduce_finalize(int n_energy, int n_bins, const double *acc, c
     if (isi && b == 0) isi[e] = (float)(total[e] * dq2);
 }
 
+// De-interleaves the paper's Real4 morphology of one material into four arrays and
+// records max |S| (as the bit pattern of a non-negative float, so an integer atomicMax orders it).
+__global__ void __launch_bounds__(256)
+k_aos_to_soa(const float4 *__restrict__ src, float *__restrict__ phi, float *__restrict__ S, float *__restrict__ theta,
+             float *__restrict__ psi, size_t n, unsigned int *max_s_bits)
+{
+    float m = 0.f;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float4 v = __ldcs(src + i);
+        phi[i] = v.x; S[i] = v.y; psi[i] = v.z; theta[i] = v.w;
+        m = fmaxf(m, fabsf(v.y));
+        if (v.y != v.y) m = __int_as_float(0x7f800000);          // NaN counts as "aligned"
+    }
+    for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_down_sync(0xffffffffu, m, d));
+    if ((threadIdx.x & 31) == 0 && m > 0.f) atomicMax(max_s_bits, __float_as_uint(m));
+}
+
 } // namespace cyr

@@ -248,3 +248,33 @@ def test_reduce_rejects_bad_arguments():
             ctx.reduce(img.data_ptr(), None, 1, bins, width, I.data_ptr())
         assert ei.value.status == binding.ERR_INVALID_ARG
     ctx.close()
+
+
+def test_aos_morphology_matches_soa():
+    """cyrsoxs_set_morphology_aos (the paper's Real4 layout): same images, bit for bit,
+    as the structure-of-arrays entry; an S == 0 material is detected as isotropic."""
+    import torch
+    from paper_2209_13121_b200 import binding
+    w = W.tiny(seed=41, nx=32, ny=16, nz=8, n_mat=3, n_energy=2, voxel_nm=2.0)
+    ref = binding.simulate(w, want_counts=True)
+    n = w.Nx * w.Ny * w.Nz
+    aos = np.zeros((w.n_mat, n, 4), np.float32)
+    for m, (phi, S, th, ps) in enumerate(w.materials):
+        aos[m, :, 0] = phi.ravel()
+        if S is not None:
+            aos[m, :, 1] = S.ravel(); aos[m, :, 2] = ps.ravel(); aos[m, :, 3] = th.ravel()
+    d = torch.from_numpy(aos).cuda()
+    ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    s = torch.cuda.current_stream().cuda_stream
+    ctx.set_morphology_aos(d.data_ptr(), s)
+    ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald)
+    out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32, device="cuda")
+    ctx.run(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref[0])
+    # the isotropic last material was detected: same transform count as the SoA run
+    assert ctx.stats()["stage_bytes"]["xpass"] == ref[-1].stats()["stage_bytes"]["xpass"]
+    with pytest.raises(binding.CyrsoxsError):
+        ctx.set_morphology_aos(0, s)
+    ctx.close()
