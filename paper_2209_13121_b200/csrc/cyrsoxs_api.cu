@@ -66,7 +66,6 @@ struct cyrsoxs_ctx {
     int profiling = 0;
     unsigned int *d_counts = nullptr;
     // SPECTRAL_BASIS plan (rebuilt per run from the morphology's NULL pattern and the optics)
-    BasisGroups groups{};
     int n_pack = 0;
     std::vector<int> basis_kind, basis_mat;     // [2 n_pack]
     DevBuf d_bcoef, d_bkind;
@@ -464,8 +463,7 @@ cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int
     return launch_rotate(c, st, e0, eb, d_out, d_cnt);
 }
 
-template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, const BasisGroups &, float2 *out,
-                                                   const Window &wx, int pitch)
+template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, float2 *out, const Window &wx, int pitch)
 {
     using Cfg = XB2Cfg<LOGN>;
     static bool attr_done[64] = {false};
@@ -481,10 +479,10 @@ template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t 
     return CYRSOXS_OK;
 }
 
-cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, const BasisGroups &g, float2 *out, const Window &wx, int pitch)
+cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, float2 *out, const Window &wx, int pitch)
 {
     switch (ilog2(c->Nx)) {
-#define CASE(L) case L: return launch_xbasis_t<L>(c, st, g, out, wx, pitch);
+#define CASE(L) case L: return launch_xbasis_t<L>(c, st, out, wx, pitch);
         CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11)
 #undef CASE
     }
@@ -496,7 +494,6 @@ cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, const BasisGroups 
 // coefficient of each field (times 1/2 for the unpacking).
 cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c)
 {
-    memset(&c->groups, 0, sizeof c->groups);
     c->basis_kind.clear(); c->basis_mat.clear();
     for (int m = 0; m < c->n_mat; ++m) {
         if (c->mp.S[m] != nullptr) for (int kd = BK_PHI; kd <= BK_YZ; ++kd) { c->basis_kind.push_back(kd); c->basis_mat.push_back(m); }
@@ -531,7 +528,6 @@ cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c)
 // Spectra of all basis packs: x -> z -> y, once per run.  A3 = [pack][wz][wy][pitch].
 cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &wx, const Window &wy, const Window &wz, int pitch)
 {
-    const BasisGroups &G = c->groups;
     const size_t rows = (size_t)c->Ny * c->Nz;
     const int F = c->n_pack;
     float2 *A1 = (float2 *)c->A1.p, *A2 = (float2 *)c->A2.p, *A3 = (float2 *)c->A3.p;
@@ -539,7 +535,7 @@ cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &
     cyrsoxs_status s;
     {
         StageTimer t(c, st, CYRSOXS_STAGE_XPASS);
-        if ((s = launch_xbasis(c, st, G, A1, wx, pitch)) != CYRSOXS_OK) return s;
+        if ((s = launch_xbasis(c, st, A1, wx, pitch)) != CYRSOXS_OK) return s;
         double n_iso = 0, n_al = 0;
         for (int m = 0; m < c->n_mat; ++m) (c->mp.S[m] ? n_al : n_iso) += 1;
         c->stats.stage_bytes[CYRSOXS_STAGE_XPASS] += nvox * (16.0 * n_al + 4.0 * n_iso) + 8.0 * F * rows * pitch;

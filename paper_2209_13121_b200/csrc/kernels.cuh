@@ -1,6 +1,6 @@
 // kernels.cuh -- the sm_100a kernels of the CyRSoXS hot path.
 //   k_xpass_chi   polarization (Eq. 2-5) fused with the FFT along x, pruned store
-//   k_colpass     strided FFT along z or y with a pruned, windowed store
+//   (k_xbasis2, k_col2p, k_col2: the SPECTRAL_BASIS x pass and the column passes, kernels2.cuh)
 //   k_ewald_chi   Ewald gather (Eq. 8) + (I - r r^T) + |.|^2 (Eq. 7) -> (I_xx, I_yy, I_xy, valid)
 //   k_rotate_avg  rotate back by -zeta (bilinear), accumulate over angles, divide by counts
 // Geometry decisions use IEEE double with explicitly rounded operations (__dmul_rn ...), the
@@ -162,133 +162,18 @@ k_xpass_chi(const __grid_constant__ MorphPtrs mp, const float *__restrict__ coef
 }
 
 // ------------------------------------------------------------------------------------------
-// x pass, SPECTRAL_BASIS algorithm (DESIGN 7.2).  p is linear in the optical constants, so
-// the energy-independent REAL fields
+// SPECTRAL_BASIS algorithm (DESIGN 7.0): p is linear in the optical constants, so the
+// energy-independent REAL fields
 //   aligned material m:  phi, w = phi S, w dx dx, w dy dy, w dx dy, w dx dz, w dy dz   (7)
 //   isotropic material:  phi                                                           (1)
-// are transformed once per run.  Two real fields share one complex transform (field 2j in
-// the real part of pack j, field 2j+1 in the imaginary part); the Ewald kernel separates them
-// with F_a(q) = (Z(q) + conj Z(-q))/2, F_b(q) = (Z(q) - conj Z(-q))/(2i).
-// Materials are split into groups of at most 16 fields (8 packs); blockIdx.y = group.
-constexpr int BASIS_MAX_FIELDS = 16;
-constexpr int BASIS_MAX_PACKS = BASIS_MAX_FIELDS / 2;
-constexpr int BASIS_MAX_GROUPS = 16;
+// are transformed once per run (k_xbasis2 in kernels2.cuh).  Two real fields share one complex
+// transform (field 2j in the real part of pack j, field 2j+1 in the imaginary part); the Ewald
+// kernel separates them with F_a(q) = (Z(q) + conj Z(-q))/2, F_b(q) = (Z(q) - conj Z(-q))/(2i).
 enum BasisKind : int { BK_NONE = 0, BK_PHI, BK_W, BK_XX, BK_YY, BK_XY, BK_XZ, BK_YZ };
 
-struct BasisGroup {
-    int n_mat;
-    int mat[BASIS_MAX_FIELDS];
-    int n_fields;                 // 7 per aligned + 1 per isotropic material
-    int pack0;                    // first pack of this group in the spectrum buffer
-};
-struct BasisGroups {
-    int n_groups;
-    BasisGroup g[BASIS_MAX_GROUPS];
-};
-
-template <int LOGN> struct XBasisCfg {
-    static constexpr int N = 1 << LOGN;
-    static constexpr int TPR = XCfg<LOGN>::TPR, ROWS = XCfg<LOGN>::ROWS, THREADS = XCfg<LOGN>::THREADS;
-    static constexpr int CHUNK = 4;                                    // packs per fft_lines call
-    static constexpr int LS = RowLayout<N>::LS;
-    static constexpr size_t SMEM = sizeof(float) * 2 * (size_t)(ROWS * BASIS_MAX_PACKS) * LS + sizeof(float2) * N;
-};
-
-template <int LOGN>
-__global__ void __launch_bounds__(XBasisCfg<LOGN>::THREADS)
-k_xpass_basis(const __grid_constant__ MorphPtrs mp, const __grid_constant__ BasisGroups groups,
-              float2 *__restrict__ out, int rows_total, Window wx, int pitch, const float2 *__restrict__ tw_g)
-{
-    using Cfg = XBasisCfg<LOGN>;
-    constexpr int N = Cfg::N, ROWS = Cfg::ROWS, LS = Cfg::LS;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float *re = reinterpret_cast<float *>(smem_raw);
-    float *im = re + ROWS * BASIS_MAX_PACKS * LS;
-    float2 *tw = reinterpret_cast<float2 *>(im + ROWS * BASIS_MAX_PACKS * LS);
-
-    const int tid = threadIdx.x;
-    const BasisGroup &G = groups.g[blockIdx.y];
-    const int row0 = blockIdx.x * ROWS;
-    const int nrows = min(ROWS, rows_total - row0);
-    const int npk = (G.n_fields + 1) >> 1;
-
-    for (int i = tid; i < N; i += Cfg::THREADS) tw[i] = tw_g[i];
-
-    const int rr = tid / Cfg::TPR, tx = tid % Cfg::TPR;
-    constexpr int NV = N >= 4 ? 4 : N;
-    int pos[NV];
-#pragma unroll
-    for (int v = 0; v < NV; ++v) pos[v] = RowLayout<N>::input_pos(4 * tx + v);
-    auto put = [&](int fi, int v, float val) {
-        float *arr = (fi & 1) ? im : re;
-        arr[((fi >> 1) * ROWS + rr) * LS + pos[v]] = val;
-    };
-    if (rr < nrows) {
-        const size_t base = (size_t)(row0 + rr) * N + 4 * tx;
-        int fi = 0;
-        for (int mi = 0; mi < G.n_mat; ++mi) {
-            const int m = G.mat[mi];
-            const bool aligned = mp.S[m] != nullptr;
-            const float4 p4 = __ldg(reinterpret_cast<const float4 *>(mp.phi[m] + base));
-            const float ph[4] = {p4.x, p4.y, p4.z, p4.w};
-            if (aligned) {
-                const float4 s4 = __ldg(reinterpret_cast<const float4 *>(mp.S[m] + base));
-                const float4 t4 = __ldg(reinterpret_cast<const float4 *>(mp.theta[m] + base));
-                const float4 q4 = __ldg(reinterpret_cast<const float4 *>(mp.psi[m] + base));
-                const float s[4] = {s4.x, s4.y, s4.z, s4.w}, th[4] = {t4.x, t4.y, t4.z, t4.w}, ps[4] = {q4.x, q4.y, q4.z, q4.w};
-#pragma unroll
-                for (int v = 0; v < NV; ++v) {
-                    const float w = ph[v] * s[v];
-                    float st, ct, sp, cp;
-                    sincosf(th[v], &st, &ct);
-                    sincosf(ps[v], &sp, &cp);
-                    const float dx = cp * st, dy = sp * st, dz = ct;
-                    const float wx_ = w * dx, wy_ = w * dy;
-                    put(fi + 0, v, ph[v]); put(fi + 1, v, w);
-                    put(fi + 2, v, wx_ * dx); put(fi + 3, v, wy_ * dy);
-                    put(fi + 4, v, wx_ * dy); put(fi + 5, v, wx_ * dz); put(fi + 6, v, wy_ * dz);
-                }
-                fi += 7;
-            } else {
-#pragma unroll
-                for (int v = 0; v < NV; ++v) put(fi, v, ph[v]);
-                fi += 1;
-            }
-        }
-        if (fi & 1) {
-#pragma unroll
-            for (int v = 0; v < NV; ++v) put(fi, v, 0.f);
-        }
-    } else {
-        // unused rows of a ragged last CTA: keep them finite
-        for (int pk = 0; pk < npk; ++pk)
-#pragma unroll
-            for (int v = 0; v < NV; ++v) { re[(pk * ROWS + rr) * LS + pos[v]] = 0.f; im[(pk * ROWS + rr) * LS + pos[v]] = 0.f; }
-    }
-    __syncthreads();
-
-    for (int c0 = 0; c0 < npk; c0 += Cfg::CHUNK) {
-        RowAcc<N> racc{re + c0 * ROWS * LS, im + c0 * ROWS * LS};
-        fft_lines<LOGN, Cfg::CHUNK * ROWS, Cfg::THREADS>(racc, min(Cfg::CHUNK, npk - c0) * ROWS, tw, tid);
-    }
-
-    const size_t fstride = (size_t)rows_total * pitch;
-    for (int idx = tid; idx < npk * nrows * pitch; idx += Cfg::THREADS) {
-        const int lr = idx / pitch, sl = idx - lr * pitch;
-        const int pk = lr / nrows, r = lr - pk * nrows;
-        float2 val = make_float2(0.f, 0.f);
-        if (sl < wx.W) {
-            const int b = (wx.lo + sl) & (N - 1);
-            const int p = (pk * ROWS + r) * LS + RowLayout<N>::pos(b);
-            val = make_float2(re[p], im[p]);
-        }
-        out[(size_t)(G.pack0 + pk) * fstride + (size_t)(row0 + r) * pitch + sl] = val;
-    }
-}
-
 // ------------------------------------------------------------------------------------------
-// Strided pass (z or y): a CTA loads a tile of N rows x TX contiguous columns, transforms the
-// TX columns, stores the rows whose bins lie in the window.  Batches: blockIdx.x = tile +
+// Strided pass (z or y), kernels in kernels2.cuh: a CTA transforms a tile of TX contiguous columns by
+// N rows and stores the rows whose bins lie in the window.  Batches: blockIdx.x = tile +
 // n_tiles * lo, blockIdx.y = hi, with separate in/out strides (in float2 units).
 struct ColParams {
     const float2 *in;
@@ -300,49 +185,6 @@ struct ColParams {
     Window win;
     const float2 *tw;
 };
-
-template <int LOGN> struct ColCfg {
-    static constexpr int N = 1 << LOGN;
-    static constexpr int TX = N >= 1024 ? 8 : (N >= 256 ? 16 : 32);
-    static constexpr int ELEMS = N * TX;
-    static constexpr int THREADS_RAW = ELEMS / 16;
-    static constexpr int THREADS = THREADS_RAW > 512 ? 512 : (THREADS_RAW < 64 ? 64 : THREADS_RAW);
-    static constexpr size_t SMEM = sizeof(float2) * ((size_t)ELEMS + N);
-};
-
-template <int LOGN>
-__global__ void __launch_bounds__(ColCfg<LOGN>::THREADS)
-k_colpass(const ColParams p)
-{
-    using Cfg = ColCfg<LOGN>;
-    constexpr int N = Cfg::N, TX = Cfg::TX, HX = TX / 2;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2 *s = reinterpret_cast<float2 *>(smem_raw);
-    float2 *tw = s + Cfg::ELEMS;
-    const int tid = threadIdx.x;
-    const int tile = blockIdx.x % p.n_tiles, lo = blockIdx.x / p.n_tiles, hi = blockIdx.y;
-
-    const float2 *src = p.in + (size_t)hi * p.in_hi + (size_t)lo * p.in_lo + (size_t)tile * TX;
-#pragma unroll 4
-    for (int idx = tid; idx < N * HX; idx += Cfg::THREADS) {
-        const int i = idx / HX, c2 = idx % HX;
-        const float4 v = __ldcs(reinterpret_cast<const float4 *>(src + (size_t)i * p.in_row + 2 * c2));
-        *reinterpret_cast<float4 *>(s + i * TX + 2 * c2) = v;
-    }
-    for (int i = tid; i < N; i += Cfg::THREADS) tw[i] = p.tw[i];
-    __syncthreads();
-
-    ColAcc<N, TX> cacc{s};
-    fft_lines<LOGN, TX, Cfg::THREADS>(cacc, TX, tw, tid);
-
-    float2 *dst = p.out + (size_t)hi * p.out_hi + (size_t)lo * p.out_lo + (size_t)tile * TX;
-    for (int idx = tid; idx < p.win.W * HX; idx += Cfg::THREADS) {
-        const int sl = idx / HX, c2 = idx % HX;
-        const int b = (p.win.lo + sl) & (N - 1);
-        const float4 v = *reinterpret_cast<const float4 *>(s + b * TX + 2 * c2);
-        *reinterpret_cast<float4 *>(dst + (size_t)sl * p.out_row + 2 * c2) = v;
-    }
-}
 
 // ------------------------------------------------------------------------------------------
 // Ewald projection.  One thread per detector pixel and energy.

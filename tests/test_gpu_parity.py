@@ -278,3 +278,32 @@ def test_aos_morphology_matches_soa():
     with pytest.raises(binding.CyrsoxsError):
         ctx.set_morphology_aos(0, s)
     ctx.close()
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_degenerate_and_extreme_cases(alg):
+    from paper_2209_13121_b200 import binding
+    # the longest supported axis along z
+    w = W.tiny(seed=51, nx=4, ny=4, nz=2048, n_mat=2, n_energy=1, voxel_nm=1.0, ewald=W.EWALD_TRILINEAR)
+    ref, rcnt = oracle_run(w)
+    out, cnt, _ = _gpu(w, alg)
+    compare(out, cnt, ref, rcnt, "nz2048")
+    # the largest material count (32: 31 aligned + 1 isotropic = 218 basis fields)
+    w = W.tiny(seed=52, nx=8, ny=8, nz=4, n_mat=32, n_energy=2, voxel_nm=3.0, ewald=W.EWALD_NEAREST)
+    ref, rcnt = oracle_run(w)
+    out, cnt, _ = _gpu(w, alg)
+    compare(out, cnt, ref, rcnt, "32-materials")
+    # more energies than one batch holds (batches of 256), 2-D
+    w = W.tiny(seed=53, nx=16, ny=8, nz=1, n_mat=2, n_energy=300, voxel_nm=4.0, energies=np.linspace(270.0, 340.0, 300))
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, ctx = _gpu(w, alg)
+    compare(out, cnt, ref, rcnt, "300-energies")
+    # an empty model (phi == 0 everywhere): every image is exactly zero, counts are pure geometry
+    z = [(np.zeros_like(m[0]), None if m[1] is None else np.zeros_like(m[1]), None if m[2] is None else np.zeros_like(m[2]),
+          None if m[3] is None else np.zeros_like(m[3])) for m in W.tiny(seed=54, nx=16, ny=16, nz=4, n_mat=2).materials]
+    w0 = W.tiny(seed=54, nx=16, ny=16, nz=4, n_mat=2)
+    w0 = W.Workload("empty", 16, 16, 4, w0.voxel_nm, z, w0.energies, w0.delta_par, w0.beta_par, w0.delta_perp, w0.beta_perp,
+                    w0.angles, w0.ewald)
+    ref, rcnt = oracle_run(w0)
+    out, cnt, _ = _gpu(w0, alg)
+    assert (out == 0).all() and (ref == 0).all() and (cnt == rcnt).all()
