@@ -119,6 +119,22 @@ cyrsoxs_status cyrsoxs_set_morphology_host(cyrsoxs_ctx *ctx, const float *const 
  * This call synchronises `cuda_stream` once (to read back the per-material max |S|). */
 cyrsoxs_status cyrsoxs_set_morphology_aos(cyrsoxs_ctx *ctx, const float *d_real4, void *cuda_stream);
 
+/* Memory-minimising variant (the idea of the paper's Algorithm 2/3: the morphology is
+ * only needed while the polarization precursor is formed, so it is streamed through the device
+ * instead of kept there).  The four tables are HOST arrays of n_mat HOST pointers (as in
+ * cyrsoxs_set_morphology_host, PINNED memory for the copies to overlap) that are BORROWED: they
+ * must stay valid and unmodified across every later cyrsoxs_run.  Each run uploads the materials
+ * `materials_per_group` (>= 1) at a time into a double-buffered device staging area of
+ * 2 * materials_per_group * 16 bytes per voxel on an internal copy stream, while the previous
+ * group's fields are transformed; the device never holds more of the morphology than that.
+ * The energy-independent spectra of SPECTRAL_BASIS play the role of the paper's N_t (they are
+ * formed once per run, not once per energy); CYRSOXS_ALG_PER_ENERGY is refused in this mode
+ * (NOT_IMPLEMENTED at cyrsoxs_run).  Results equal the resident mode's within rounding (fields
+ * are paired inside a group, so the pairing can differ). */
+cyrsoxs_status cyrsoxs_set_morphology_streamed(cyrsoxs_ctx *ctx, const float *const *h_phi,
+                                               const float *const *h_S, const float *const *h_theta,
+                                               const float *const *h_psi, int materials_per_group);
+
 /* Energy list and the material library: HOST arrays, copied.  energies_eV has
  * n_energy entries (> 0); the four tables are [n_energy][n_mat] float32 with
  * n_par = 1 - delta_par + i beta_par, n_perp likewise.  The complex coefficients

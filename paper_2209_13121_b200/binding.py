@@ -19,7 +19,7 @@ STAGES = ("xpass", "zpass", "ypass", "ewald", "rotate")
 N_STAGES = len(STAGES)
 
 EXPORTS = [
-    "cyrsoxs_create", "cyrsoxs_set_morphology", "cyrsoxs_set_morphology_host", "cyrsoxs_set_morphology_aos",
+    "cyrsoxs_create", "cyrsoxs_set_morphology", "cyrsoxs_set_morphology_host", "cyrsoxs_set_morphology_aos", "cyrsoxs_set_morphology_streamed",
     "cyrsoxs_set_optical_constants", "cyrsoxs_set_angles", "cyrsoxs_set_ewald", "cyrsoxs_set_algorithm",
     "cyrsoxs_set_counts_output", "cyrsoxs_set_profiling", "cyrsoxs_run", "cyrsoxs_num_angles",
     "cyrsoxs_get_stats", "cyrsoxs_reduce", "cyrsoxs_debug_fetch_images", "cyrsoxs_last_error", "cyrsoxs_destroy",
@@ -59,6 +59,7 @@ def load() -> C.CDLL:
     lib.cyrsoxs_set_morphology.argtypes = [vp, fpp, fpp, fpp, fpp]
     lib.cyrsoxs_set_morphology_host.argtypes = [vp, fpp, fpp, fpp, fpp, vp]
     lib.cyrsoxs_set_morphology_aos.argtypes = [vp, vp, vp]
+    lib.cyrsoxs_set_morphology_streamed.argtypes = [vp, fpp, fpp, fpp, fpp, C.c_int]
     lib.cyrsoxs_set_optical_constants.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp]
     lib.cyrsoxs_set_angles.argtypes = [vp, C.c_double, C.c_double, C.c_double]
     lib.cyrsoxs_set_ewald.argtypes = [vp, C.c_int]
@@ -135,8 +136,7 @@ class Context:
         self._check(self.lib.cyrsoxs_set_morphology(self.h, *tabs))
         self._keep = keep
 
-    def set_morphology_host(self, materials, stream: int = 0):
-        """materials: list of (phi, S, theta, psi) host arrays (numpy or pinned torch), copied by the library."""
+    def _host_tables(self, materials):
         tabs = []
         keep = []
         for k in range(4):
@@ -150,7 +150,19 @@ class Context:
                 else:
                     keep.append(t); col.append(t.ctypes.data)
             tabs.append(_table(col))
+        return tabs, keep
+
+    def set_morphology_host(self, materials, stream: int = 0):
+        """materials: list of (phi, S, theta, psi) host arrays (numpy or pinned torch), copied by the library."""
+        tabs, keep = self._host_tables(materials)
         self._check(self.lib.cyrsoxs_set_morphology_host(self.h, *tabs, C.c_void_p(stream)))
+        self._keep = keep
+
+    def set_morphology_streamed(self, materials, materials_per_group: int = 1):
+        """materials: list of (phi, S, theta, psi) pinned host arrays, BORROWED for every later run: the
+        morphology is streamed through a 2 x materials_per_group staging area at each run."""
+        tabs, keep = self._host_tables(materials)
+        self._check(self.lib.cyrsoxs_set_morphology_streamed(self.h, *tabs, int(materials_per_group)))
         self._keep = keep
 
     def set_morphology_aos(self, real4_ptr: int, stream: int = 0):

@@ -43,6 +43,12 @@ struct cyrsoxs_ctx {
     MorphPtrs mp{};
     bool have_morph = false;
     std::vector<void *> owned_morph;
+    // streamed mode (cyrsoxs_set_morphology_streamed): host arrays, group size, staging, events
+    bool streamed = false;
+    int stream_group = 0;
+    MorphPtrs host_mp{};
+    DevBuf stage_morph[2];
+    cudaEvent_t ev_stage_ready[2] = {nullptr, nullptr}, ev_stage_free[2] = {nullptr, nullptr};
     // optics
     int nE = 0;
     std::vector<double> energies, k;
@@ -463,7 +469,7 @@ cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int
     return launch_rotate(c, st, e0, eb, d_out, d_cnt);
 }
 
-template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, float2 *out, const Window &wx, int pitch)
+template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch)
 {
     using Cfg = XB2Cfg<LOGN>;
     static bool attr_done[64] = {false};
@@ -474,20 +480,23 @@ template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t 
     }
     const int rows = c->Ny * c->Nz;
     dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS);
-    k_xbasis2<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(c->mp, out, rows, wx, pitch, (const float2 *)c->twx.p);
+    k_xbasis2<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(mp, out, rows, wx, pitch, (const float2 *)c->twx.p);
     CUDA_TRY(c, cudaGetLastError());
     return CYRSOXS_OK;
 }
 
-cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, float2 *out, const Window &wx, int pitch)
+cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch)
 {
     switch (ilog2(c->Nx)) {
-#define CASE(L) case L: return launch_xbasis_t<L>(c, st, out, wx, pitch);
+#define CASE(L) case L: return launch_xbasis_t<L>(c, st, mp, out, wx, pitch);
         CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11)
 #undef CASE
     }
     return fail(c, CYRSOXS_ERR_INVALID_ARG, "unsupported Nx");
 }
+
+// Is material m aligned (has S, theta, psi)?  In streamed mode the host table decides.
+bool is_aligned(const cyrsoxs_ctx *c, int m) { return (c->streamed ? c->host_mp.S[m] : c->mp.S[m]) != nullptr; }
 
 // The basis fields in material order (7 per aligned, 1 per isotropic material), two per complex
 // pack, the last pack padded; the per-field kind/material tables and the per-energy complex
@@ -496,8 +505,12 @@ cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c)
 {
     c->basis_kind.clear(); c->basis_mat.clear();
     for (int m = 0; m < c->n_mat; ++m) {
-        if (c->mp.S[m] != nullptr) for (int kd = BK_PHI; kd <= BK_YZ; ++kd) { c->basis_kind.push_back(kd); c->basis_mat.push_back(m); }
+        if (is_aligned(c, m)) for (int kd = BK_PHI; kd <= BK_YZ; ++kd) { c->basis_kind.push_back(kd); c->basis_mat.push_back(m); }
         else { c->basis_kind.push_back(BK_PHI); c->basis_mat.push_back(m); }
+        // streamed mode: every material group is transformed by its own launch, so its fields are
+        // paired among themselves and an odd count is padded at the group's end
+        const bool group_end = c->streamed && ((m + 1) % c->stream_group == 0);
+        if (group_end && (c->basis_kind.size() & 1)) { c->basis_kind.push_back(BK_NONE); c->basis_mat.push_back(0); }
     }
     if (c->basis_kind.size() & 1) { c->basis_kind.push_back(BK_NONE); c->basis_mat.push_back(0); }
     const int pack = (int)c->basis_kind.size() / 2;
@@ -533,13 +546,56 @@ cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &
     float2 *A1 = (float2 *)c->A1.p, *A2 = (float2 *)c->A2.p, *A3 = (float2 *)c->A3.p;
     const double nvox = (double)c->Nx * c->Ny * c->Nz;
     cyrsoxs_status s;
-    {
+    double n_iso = 0, n_al = 0;
+    for (int m = 0; m < c->n_mat; ++m) (is_aligned(c, m) ? n_al : n_iso) += 1;
+    if (!c->streamed) {
         StageTimer t(c, st, CYRSOXS_STAGE_XPASS);
-        if ((s = launch_xbasis(c, st, A1, wx, pitch)) != CYRSOXS_OK) return s;
-        double n_iso = 0, n_al = 0;
-        for (int m = 0; m < c->n_mat; ++m) (c->mp.S[m] ? n_al : n_iso) += 1;
-        c->stats.stage_bytes[CYRSOXS_STAGE_XPASS] += nvox * (16.0 * n_al + 4.0 * n_iso) + 8.0 * F * rows * pitch;
+        if ((s = launch_xbasis(c, st, c->mp, A1, wx, pitch)) != CYRSOXS_OK) return s;
+    } else {
+        // Memory-minimising mode (the paper's Algorithm 2/3 idea): material groups are
+        // uploaded into a double-buffered staging area on the copy stream while the previous group's
+        // fields are transformed on `st`; the spectra play the role of N_t.
+        const size_t nv = (size_t)c->Nx * c->Ny * c->Nz, abytes = sizeof(float) * nv;
+        const int G = c->stream_group;
+        if (!c->copy_stream) CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            if ((s = ensure(c, c->stage_morph[i], abytes * 4 * (size_t)G)) != CYRSOXS_OK) return s;
+            if (!c->ev_stage_ready[i]) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_stage_ready[i], cudaEventDisableTiming));
+            if (!c->ev_stage_free[i]) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_stage_free[i], cudaEventDisableTiming));
+        }
+        const size_t fstride = rows * (size_t)pitch;
+        int pack0 = 0, g = 0;
+        for (int m0 = 0; m0 < c->n_mat; m0 += G, ++g) {
+            const int slot = g & 1, m1 = std::min(c->n_mat, m0 + G);
+            // the slot is free once the x pass that last read it (two groups ago, or in the previous run) is done
+            CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_stage_free[slot], 0));
+            MorphPtrs sub{};
+            sub.n_mat = m1 - m0;
+            float *base = (float *)c->stage_morph[slot].p;
+            int fields = 0;
+            for (int m = m0; m < m1; ++m) {
+                const float *src[4] = {c->host_mp.phi[m], c->host_mp.S[m], c->host_mp.theta[m], c->host_mp.psi[m]};
+                const float *dst[4] = {nullptr, nullptr, nullptr, nullptr};
+                for (int j = 0; j < 4; ++j) {
+                    if (!src[j]) continue;
+                    float *d = base + ((size_t)(m - m0) * 4 + j) * nv;
+                    CUDA_TRY(c, cudaMemcpyAsync(d, src[j], abytes, cudaMemcpyHostToDevice, c->copy_stream));
+                    dst[j] = d;
+                }
+                sub.phi[m - m0] = dst[0]; sub.S[m - m0] = dst[1]; sub.theta[m - m0] = dst[2]; sub.psi[m - m0] = dst[3];
+                fields += src[1] ? 7 : 1;
+            }
+            CUDA_TRY(c, cudaEventRecord(c->ev_stage_ready[slot], c->copy_stream));
+            CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_stage_ready[slot], 0));
+            {
+                StageTimer t(c, st, CYRSOXS_STAGE_XPASS);
+                if ((s = launch_xbasis(c, st, sub, A1 + (size_t)pack0 * fstride, wx, pitch)) != CYRSOXS_OK) return s;
+            }
+            CUDA_TRY(c, cudaEventRecord(c->ev_stage_free[slot], st));
+            pack0 += (fields + 1) / 2;
+        }
     }
+    c->stats.stage_bytes[CYRSOXS_STAGE_XPASS] += nvox * (16.0 * n_al + 4.0 * n_iso) + 8.0 * F * rows * pitch;
     const float2 *ysrc = A1;
     if (c->Nz > 1) {
         StageTimer t(c, st, CYRSOXS_STAGE_ZPASS);
@@ -639,6 +695,11 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
     for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->d_tiles[4], &c->d_tiles[5], &c->d_tiles[6], &c->d_tiles[7], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
                       &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind, &c->red})
         release(*b);
+    release(c->stage_morph[0]); release(c->stage_morph[1]);
+    for (int i = 0; i < 2; ++i) {
+        if (c->ev_stage_ready[i]) cudaEventDestroy(c->ev_stage_ready[i]);
+        if (c->ev_stage_free[i]) cudaEventDestroy(c->ev_stage_free[i]);
+    }
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     for (int i = 0; i < 2; ++i) {
         if (c->ev_batch[i]) cudaEventDestroy(c->ev_batch[i]);
@@ -650,7 +711,8 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
 static void note_null_pattern(cyrsoxs_ctx *c)
 {
     unsigned long long pat = 0;
-    for (int m = 0; m < c->n_mat; ++m) pat |= (unsigned long long)(c->mp.S[m] != nullptr) << m;
+    for (int m = 0; m < c->n_mat; ++m) pat |= (unsigned long long)is_aligned(c, m) << m;
+    if (c->streamed) pat ^= 0x8000000000000000ull ^ ((unsigned long long)c->stream_group << 40);
     if (pat != c->null_pattern) { c->null_pattern = pat; c->plan_dirty = true; }
 }
 
@@ -684,6 +746,7 @@ cyrsoxs_status cyrsoxs_set_morphology(cyrsoxs_ctx *c, const float *const *d_phi,
         c->mp.theta[m] = d_theta ? d_theta[m] : nullptr;
         c->mp.psi[m] = d_psi ? d_psi[m] : nullptr;
     }
+    c->streamed = false;
     note_null_pattern(c);
     c->have_morph = true;
     return CYRSOXS_OK;
@@ -736,6 +799,32 @@ cyrsoxs_status cyrsoxs_set_morphology_host(cyrsoxs_ctx *c, const float *const *h
         c->mp.phi[m] = dptr[4 * m]; c->mp.S[m] = dptr[4 * m + 1];
         c->mp.theta[m] = dptr[4 * m + 2]; c->mp.psi[m] = dptr[4 * m + 3];
     }
+    c->streamed = false;
+    note_null_pattern(c);
+    c->have_morph = true;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_morphology_streamed(cyrsoxs_ctx *c, const float *const *h_phi, const float *const *h_S,
+                                               const float *const *h_theta, const float *const *h_psi, int materials_per_group)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    cyrsoxs_status st = check_morph_tables(c, h_phi, h_S, h_theta, h_psi);
+    if (st != CYRSOXS_OK) return st;
+    if (materials_per_group < 1) return fail(c, CYRSOXS_ERR_INVALID_ARG, "materials_per_group must be >= 1");
+    for (int m = 0; m < c->n_mat; ++m) {
+        c->host_mp.phi[m] = h_phi[m];
+        c->host_mp.S[m] = h_S ? h_S[m] : nullptr;
+        c->host_mp.theta[m] = h_theta ? h_theta[m] : nullptr;
+        c->host_mp.psi[m] = h_psi ? h_psi[m] : nullptr;
+        c->mp.phi[m] = c->mp.S[m] = c->mp.theta[m] = c->mp.psi[m] = nullptr;
+    }
+    c->host_mp.n_mat = c->n_mat;
+    c->streamed = true;
+    c->stream_group = std::min(materials_per_group, c->n_mat);
+    for (void *p : c->owned_morph) cudaFree(p);
+    c->owned_morph.clear();
+    c->plan_dirty = true;
     note_null_pattern(c);
     c->have_morph = true;
     return CYRSOXS_OK;
@@ -787,6 +876,7 @@ cyrsoxs_status cyrsoxs_set_morphology_aos(cyrsoxs_ctx *c, const float *d_real4, 
         c->mp.theta[m] = aligned ? (const float *)c->owned_morph[4 * m + 2] : nullptr;
         c->mp.psi[m] = aligned ? (const float *)c->owned_morph[4 * m + 3] : nullptr;
     }
+    c->streamed = false;
     note_null_pattern(c);
     c->have_morph = true;
     return CYRSOXS_OK;
@@ -941,7 +1031,9 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     // (register-first x pass, real fields) costs about half of a PER_ENERGY one (measured on cfg3: 0.31 ms
     // per pack against 0.6 ms per field), hence the factor 2
     int alg = c->alg;
-    if (alg == CYRSOXS_ALG_AUTO) alg = (2 * NCHI * c->nE >= c->n_pack) ? CYRSOXS_ALG_SPECTRAL_BASIS : CYRSOXS_ALG_PER_ENERGY;
+    if (alg == CYRSOXS_ALG_AUTO) alg = (c->streamed || 2 * NCHI * c->nE >= c->n_pack) ? CYRSOXS_ALG_SPECTRAL_BASIS : CYRSOXS_ALG_PER_ENERGY;
+    if (c->streamed && alg != CYRSOXS_ALG_SPECTRAL_BASIS)
+        return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "a streamed morphology needs CYRSOXS_ALG_SPECTRAL_BASIS (or AUTO)");
     const bool spectral = alg == CYRSOXS_ALG_SPECTRAL_BASIS;
 
     // plan: windows for the largest k, energy batch from the free memory

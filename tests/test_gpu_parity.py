@@ -307,3 +307,42 @@ def test_degenerate_and_extreme_cases(alg):
     ref, rcnt = oracle_run(w0)
     out, cnt, _ = _gpu(w0, alg)
     assert (out == 0).all() and (ref == 0).all() and (cnt == rcnt).all()
+
+
+@pytest.mark.parametrize("group", [1, 2, 5])
+def test_streamed_morphology_matches_oracle(group):
+    """cyrsoxs_set_morphology_streamed (NEXT-3, the paper's Algorithm 2/3 idea): materials pass through
+    a double-buffered staging area group by group; images within the gates, counts equal, and repeated
+    runs (staging slots reused across runs) give identical images."""
+    import torch
+    from paper_2209_13121_b200 import binding
+    w = W.tiny(seed=61, nx=32, ny=32, nz=8, n_mat=4, n_energy=3, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR)
+    ref, rcnt = oracle_run(w)
+    pinned = [tuple(None if a is None else torch.from_numpy(a).pin_memory() for a in m) for m in w.materials]
+    ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    ctx.set_morphology_streamed(pinned, group)
+    ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald)
+    out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32, device="cuda")
+    cnt = torch.zeros((w.n_energy, w.Ny, w.Nx), dtype=torch.int32, device="cuda")
+    ctx.set_counts_output(cnt.data_ptr())
+    s = torch.cuda.current_stream().cuda_stream
+    ctx.run(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    first = out.clone()
+    compare(out.cpu().numpy(), cnt.cpu().numpy(), ref, rcnt, f"streamed g={group}")
+    for _ in range(3):
+        ctx.run(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    assert torch.equal(out, first)
+    ctx.set_algorithm(binding.ALG_PER_ENERGY)
+    with pytest.raises(binding.CyrsoxsError) as ei:
+        ctx.run(out.data_ptr(), s)
+    assert ei.value.status == binding.ERR_NOT_IMPLEMENTED
+    # back to a resident morphology on the same context
+    ctx.set_algorithm(binding.ALG_AUTO)
+    ctx.set_morphology_host(w.materials, s)
+    ctx.run(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    compare(out.cpu().numpy(), cnt.cpu().numpy(), ref, rcnt, "resident after streamed")
+    ctx.close()
