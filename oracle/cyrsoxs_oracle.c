@@ -172,11 +172,28 @@ static cplx *make_twiddles(int n)
 
 static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
 
+/* Eq. 6 along one axis written out as the definition, O(n^2), for a length that is not a
+ * power of two (the paper uses Nz = 63; DESIGN.md 3-A14): X[k] = sum_j x[j] exp(-2 pi i
+ * j k / n).  The phase index j k mod n is exact integer arithmetic. */
+static void dft1d_definition(cplx *x, int n, cplx *scratch)
+{
+    for (int k = 0; k < n; ++k) {
+        cplx acc = 0.0;
+        for (int j = 0; j < n; ++j) {
+            double ang = -2.0 * ORC_PI * (double)(((int64_t)j * k) % n) / (double)n;
+            acc += x[j] * (cos(ang) + I * sin(ang));
+        }
+        scratch[k] = acc;
+    }
+    memcpy(x, scratch, sizeof(cplx) * (size_t)n);
+}
+
 /* 3-D FFT of f[z][y][x] (x fastest), in place: Eq. 6, forward,
- * unnormalised, origin at voxel 0.  Returns 0, or -1 if a size is not 2^k. */
+ * unnormalised, origin at voxel 0.  Nx and Ny must be powers of two (returns -1 otherwise);
+ * Nz may be any length: a power of two takes the radix-2 FFT, anything else the definition. */
 int orc_fft3(int Nx, int Ny, int Nz, cplx *f)
 {
-    if (!is_pow2(Nx) || !is_pow2(Ny) || !is_pow2(Nz)) return -1;
+    if (!is_pow2(Nx) || !is_pow2(Ny) || Nz < 1) return -1;
     const int64_t sxy = (int64_t)Nx * Ny;
     cplx *twx = make_twiddles(Nx), *twy = make_twiddles(Ny), *twz = make_twiddles(Nz);
     /* along x: contiguous rows */
@@ -205,12 +222,13 @@ int orc_fft3(int Nx, int Ny, int Nz, cplx *f)
     if (Nz > 1) {
 #pragma omp parallel
         {
-            cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)Nz);
+            cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)Nz * 2);
 #pragma omp for schedule(static)
             for (int64_t r = 0; r < sxy; ++r) {
                 cplx *base = f + r;
                 for (int z = 0; z < Nz; ++z) buf[z] = base[(int64_t)z * sxy];
-                fft1d_radix2(buf, Nz, twz);
+                if (is_pow2(Nz)) fft1d_radix2(buf, Nz, twz);
+                else dft1d_definition(buf, Nz, buf + Nz);
                 for (int z = 0; z < Nz; ++z) base[(int64_t)z * sxy] = buf[z];
             }
             free(buf);
@@ -531,7 +549,7 @@ int orc_run_energy(int Nx, int Ny, int Nz, int n_mat, double voxel,
 {
     const int64_t n_vox = (int64_t)Nx * Ny * Nz, n_pix = (int64_t)Nx * Ny;
     int n_ang = orc_num_angles(start_deg, step_deg, end_deg);
-    if (n_ang < 1 || !is_pow2(Nx) || !is_pow2(Ny) || !is_pow2(Nz)) return -1;
+    if (n_ang < 1 || !is_pow2(Nx) || !is_pow2(Ny) || Nz < 1) return -1;
     double k = orc_wavenumber(energy_eV);
     double *a = malloc(sizeof(double) * 2 * n_mat), *b = malloc(sizeof(double) * 2 * n_mat),
            *c = malloc(sizeof(double) * 2 * n_mat);
@@ -574,7 +592,7 @@ int orc_run_energy_linear(int Nx, int Ny, int Nz, int n_mat, double voxel,
 {
     const int64_t n_vox = (int64_t)Nx * Ny * Nz, n_pix = (int64_t)Nx * Ny;
     int n_ang = orc_num_angles(start_deg, step_deg, end_deg);
-    if (n_ang < 1 || !is_pow2(Nx) || !is_pow2(Ny) || !is_pow2(Nz)) return -1;
+    if (n_ang < 1 || !is_pow2(Nx) || !is_pow2(Ny) || Nz < 1) return -1;
     double k = orc_wavenumber(energy_eV);
     double *a = malloc(sizeof(double) * 2 * n_mat), *b = malloc(sizeof(double) * 2 * n_mat),
            *c = malloc(sizeof(double) * 2 * n_mat);

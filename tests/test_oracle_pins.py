@@ -540,3 +540,26 @@ def test_A6_common_rotation_leaves_X_unchanged():
         U = np.array([[np.cos(z), -np.sin(z), 0], [np.sin(z), np.cos(z), 0], [0, 0, 1]])
         X = lambda v, r: np.linalg.norm(v - r * (r @ v)) ** 2
         assert abs(X(v, r) - X(U.T @ v, U.T @ r)) < 1e-13 * X(v, r)
+
+
+def test_A14_any_Nz_definition_dft_along_z():
+    """Nz that is not a power of two (the paper uses Nz = 63; DESIGN.md 3-A14): the oracle takes the
+    definition along z.  Pins: the brute-force 3-D DFT, Parseval, and the whole pipeline with the brute-force
+    DFT swapped in, on 8 x 4 x 7 and 4 x 4 x 12."""
+    rng = np.random.default_rng(5)
+    for shape in [(7, 4, 8), (12, 4, 4), (63, 2, 4)]:
+        f = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+        F = oracle.fft3(f)
+        assert np.allclose(F, oracle.dft3_naive(f), rtol=0, atol=1e-11 * np.abs(F).max())
+        assert np.isclose((np.abs(F) ** 2).sum(), f.size * (np.abs(f) ** 2).sum(), rtol=1e-12)
+    # a single plane wave along z lands in exactly one bin, with the forward sign
+    nz, m = 7, 3
+    z = np.arange(nz).reshape(nz, 1, 1)
+    f = np.exp(2j * np.pi * m * z / nz) * np.ones((nz, 4, 4))
+    F = oracle.fft3(f)
+    assert np.isclose(F[m, 0, 0], nz * 16) and np.abs(np.delete(F[:, 0, 0], m)).max() < 1e-10
+    # whole pipeline: linear mode equals definition mode at an odd depth
+    w = W.tiny(seed=77, nx=8, ny=8, nz=7, n_mat=2, n_energy=1, voxel_nm=1.5, ewald=W.EWALD_TRILINEAR)
+    a, ca = _run(w)
+    b, cb = _run(w, linear=True)
+    assert np.array_equal(ca, cb) and np.allclose(a, b, rtol=1e-11, atol=1e-14 * a.max())
