@@ -27,6 +27,7 @@ constexpr double kPi = 3.141592653589793;
 constexpr double kHcEvNm = 1239.84197;
 constexpr int kMaxAngles = 4096;
 constexpr int kMaxLog2 = 11;
+constexpr int kMaxNzAny = 512;         // longest z axis that is not a power of two (direct DFT pass)
 
 struct DevBuf {
     void *p = nullptr;
@@ -149,8 +150,8 @@ cyrsoxs_status make_twiddles(cyrsoxs_ctx *c, DevBuf &b, int N)
         h[t] = make_float2((float)cos(ang), (float)sin(ang));
     }
     // exact values on the axes
-    if (N >= 4) { h[N / 4] = make_float2(0.f, -1.f); h[N / 2] = make_float2(-1.f, 0.f); h[3 * N / 4] = make_float2(0.f, 1.f); }
-    else if (N == 2) h[1] = make_float2(-1.f, 0.f);
+    if (N >= 4 && N % 4 == 0) { h[N / 4] = make_float2(0.f, -1.f); h[N / 2] = make_float2(-1.f, 0.f); h[3 * N / 4] = make_float2(0.f, 1.f); }
+    else if (N % 2 == 0 && N >= 2) h[N / 2] = make_float2(-1.f, 0.f);
     cyrsoxs_status st = ensure(c, b, sizeof(float2) * h.size());
     if (st != CYRSOXS_OK) return st;
     CUDA_TRY(c, cudaMemcpy(b.p, h.data(), sizeof(float2) * h.size(), cudaMemcpyHostToDevice));
@@ -288,6 +289,22 @@ template <int LOGN, int PW> cyrsoxs_status launch_colpass_pair_t(cyrsoxs_ctx *c,
 
 cyrsoxs_status launch_colpass(cyrsoxs_ctx *c, cudaStream_t st, int N, const ColParams &p, int n_lo, int n_hi, int pitch)
 {
+    if (!is_pow2(N)) {
+        // a z axis of any length (DESIGN 3-A14): the pruned direct DFT
+        const size_t smem = sizeof(float2) * ((size_t)N * DFT_TX + N);
+        static bool attr_done[64] = {false};
+        if (!attr_done[c->device & 63]) {
+            CUDA_TRY(c, cudaFuncSetAttribute(k_coldft, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)(sizeof(float2) * ((size_t)kMaxNzAny * DFT_TX + kMaxNzAny))));
+            attr_done[c->device & 63] = true;
+        }
+        ColParams q = p;
+        q.n_tiles = pitch / DFT_TX;
+        dim3 grid((unsigned)(q.n_tiles * n_lo), (unsigned)n_hi);
+        k_coldft<<<grid, DFT_TX * DFT_OG, smem, st>>>(q, N);
+        CUDA_TRY(c, cudaGetLastError());
+        return CYRSOXS_OK;
+    }
     // lengths 128 .. 1024 take the two-columns-per-thread kernel (measured faster at every one of them:
     // cfg2 z 29 -> 25 us, cfg3 z 0.75 -> 0.65 / y 0.49 -> 0.40 ms, cfg5 z 7.4 -> 4.5 / y 4.1 -> 3.1 ms)
     static const int pair_min = getenv("CYRSOXS_PAIR_MIN") ? atoi(getenv("CYRSOXS_PAIR_MIN")) : 7;      // tuning aid
@@ -664,8 +681,9 @@ cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm,
     if (!out) return CYRSOXS_ERR_INVALID_ARG;
     *out = nullptr;
     const int maxn = 1 << kMaxLog2;
-    if (!is_pow2(Nx) || !is_pow2(Ny) || !is_pow2(Nz) || Nx < 4 || Ny < 2 || Nz < 1 || Nx > maxn || Ny > maxn || Nz > maxn)
+    if (!is_pow2(Nx) || !is_pow2(Ny) || Nx < 4 || Ny < 2 || Nz < 1 || Nx > maxn || Ny > maxn || Nz > maxn)
         return CYRSOXS_ERR_INVALID_ARG;
+    if (!is_pow2(Nz) && Nz > kMaxNzAny) return CYRSOXS_ERR_INVALID_ARG;      // DESIGN 3-A14
     if (n_mat < 1 || n_mat > MAX_MAT || !(voxel_nm > 0.f) || !isfinite(voxel_nm)) return CYRSOXS_ERR_INVALID_ARG;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CYRSOXS_ERR_CUDA; }

@@ -19,7 +19,14 @@ constexpr int MAX_MAT = 32;
 struct Window {
     int N, lo, W;
 };
-__host__ __device__ __forceinline__ int win_slot(const Window &w, int k) { return (k - w.lo) & (w.N - 1); }
+// (N a power of two for x and y; the z axis may have any length, DESIGN 3-A14)
+__host__ __device__ __forceinline__ int win_slot(const Window &w, int k)
+{
+    const int d = k - w.lo;
+    if ((w.N & (w.N - 1)) == 0) return d & (w.N - 1);
+    const int r = d % w.N;
+    return r < 0 ? r + w.N : r;
+}
 
 struct MorphPtrs {
     const float *phi[MAX_MAT];

@@ -137,6 +137,44 @@ k_col2p(const ColParams p)
     }
 }
 
+// Strided pass for a length that is not a power of two (the z axis only: the paper uses Nz = 63,
+// P:459): the definition of Eq. 6 evaluated directly, and only at the window's bins -- the "direct DFT
+// at the k_z bins the Ewald pixels need" north_star allows.  A CTA stages a tile of 32 columns by N rows
+// and the twiddle table in shared memory; thread (c, og) accumulates bins s = og, og + 8, ... of column c.
+// The phase index k z mod N is stepped in exact integer arithmetic.  O(W N) per column: meant for the
+// short z axes of thin films (N <= 512), not as a general FFT.
+constexpr int DFT_TX = 32, DFT_OG = 8;
+
+__global__ void __launch_bounds__(DFT_TX * DFT_OG)
+k_coldft(const ColParams p, int N)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw);       // [N][32]
+    float2 *tw = sm + (size_t)N * DFT_TX;                     // [N]
+    const int tid = threadIdx.x, c = tid % DFT_TX, og = tid / DFT_TX;
+    const int tile = blockIdx.x % p.n_tiles, lo = blockIdx.x / p.n_tiles, hi = blockIdx.y;
+    const float2 *src = p.in + (size_t)hi * p.in_hi + (size_t)lo * p.in_lo + (size_t)tile * DFT_TX + c;
+    for (int z = og; z < N; z += DFT_OG) sm[z * DFT_TX + c] = __ldcs(src + (size_t)z * p.in_row);
+    for (int i = tid; i < N; i += DFT_TX * DFT_OG) tw[i] = p.tw[i];
+    __syncthreads();
+    float2 *dst = p.out + (size_t)hi * p.out_hi + (size_t)lo * p.out_lo + (size_t)tile * DFT_TX + c;
+    for (int sl = og; sl < p.win.W; sl += DFT_OG) {
+        int k = (p.win.lo + sl) % N;
+        if (k < 0) k += N;
+        float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
+        int idx = 0;
+        int z = 0;
+        for (; z + 1 < N; z += 2) {
+            a0 = cfma(sm[z * DFT_TX + c], tw[idx], a0);
+            idx += k; if (idx >= N) idx -= N;
+            a1 = cfma(sm[(z + 1) * DFT_TX + c], tw[idx], a1);
+            idx += k; if (idx >= N) idx -= N;
+        }
+        if (z < N) a0 = cfma(sm[z * DFT_TX + c], tw[idx], a0);
+        dst[(size_t)sl * p.out_row] = make_float2(a0.x + a1.x, a0.y + a1.y);
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // x pass of SPECTRAL_BASIS (DESIGN 7.2).  The energy-independent real fields, in material order
 //   aligned material:   phi, w = phi S, w dx dx, w dy dy, w dx dy, w dx dz, w dy dz      (7)

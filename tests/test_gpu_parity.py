@@ -24,7 +24,7 @@ def _gpu(w, alg, images=False):
 
 @pytest.mark.parametrize("alg", ALGS)
 @pytest.mark.parametrize("mode", [W.EWALD_NEAREST, W.EWALD_TRILINEAR])
-@pytest.mark.parametrize("shape", [(8, 8, 4), (32, 16, 8), (16, 64, 2), (64, 32, 1), (4, 4, 16), (16, 512, 2), (8, 4, 512), (1024, 4, 1), (8, 128, 256), (4, 1024, 2)])
+@pytest.mark.parametrize("shape", [(8, 8, 4), (32, 16, 8), (16, 64, 2), (64, 32, 1), (4, 4, 16), (16, 512, 2), (8, 4, 512), (1024, 4, 1), (8, 128, 256), (4, 1024, 2), (16, 16, 7), (32, 16, 63), (8, 8, 12), (8, 4, 3), (8, 4, 500)])
 def test_tiny_random(shape, mode, alg):
     nx, ny, nz = shape
     w = W.tiny(seed=100 + nx + nz, nx=nx, ny=ny, nz=nz, n_mat=3, n_energy=3, voxel_nm=2.0, ewald=mode)
@@ -346,3 +346,14 @@ def test_streamed_morphology_matches_oracle(group):
     torch.cuda.synchronize()
     compare(out.cpu().numpy(), cnt.cpu().numpy(), ref, rcnt, "resident after streamed")
     ctx.close()
+
+
+@pytest.mark.parametrize("alg", ALGS)
+def test_thin_film_nz63(alg):
+    """A z axis that is not a power of two, as in the paper's validation model (Nz = 63): 128 x 128 x 63
+    voxels, three materials, trilinear Ewald; the z pass is the pruned direct DFT."""
+    w = W.tiny(seed=71, nx=128, ny=128, nz=63, n_mat=3, n_energy=3, voxel_nm=1.0, ewald=W.EWALD_TRILINEAR,
+               angles=(0.0, 15.0, 165.0))
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, _ = _gpu(w, alg)
+    print("nz63", compare(out, cnt, ref, rcnt, "nz63"))
