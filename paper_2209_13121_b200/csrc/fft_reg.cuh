@@ -48,8 +48,14 @@ template <> struct RSched<11> { static constexpr int NST = 4; static constexpr i
 //            flipped for odd i >> 3; for TX = 4 bits 0..1 are XORed with bits 3..4.
 struct RowMap {
     __device__ __forceinline__ static int at(int i) { return i ^ ((i >> 3) & 15); }
+    // at(i + c) from a = at(i) for a compile-time offset c that is a multiple of 64: the swizzle reads
+    // bits 3..6 and writes bits 0..3, so a multiple of 128 commutes with it and an odd multiple of 64
+    // flips bit 6, i.e. toggles bit 3 of the mask.  Saves the shift/and/xor per access.
+    static constexpr bool kSwizzled = true;
+    __device__ __forceinline__ static int shifted(int a, int c) { return ((c & 64) ? (a ^ 8) : a) + c; }
 };
 template <int TX> struct ColMap {
+    static constexpr bool kSwizzled = false;
     __device__ __forceinline__ static int at(int i)
     {
         if (TX >= 16) return i * TX;
@@ -61,6 +67,7 @@ template <int TX> struct ColMap {
 // Pairs of lines as float4: PW pairs side by side, element i of pair c at (i PW + c).  With PW = 8 a
 // quarter-warp (one 128-bit wavefront) covers one full 128-byte row, so no swizzle is needed.
 template <int PW> struct PairMap {
+    static constexpr bool kSwizzled = false;
     __device__ __forceinline__ static int at(int i) { return i * PW; }
 };
 
@@ -110,8 +117,14 @@ template <int LOGN, class Map> struct RegFft {
 #pragma unroll
         for (int b = 0; b < B; ++b) {
             const int j = li + b * T;
+            if constexpr (Map::kSwizzled && (N / R) % 64 == 0) {
+                const int a = Map::at(j);
 #pragma unroll
-            for (int s = 0; s < R; ++s) v[b * R + s] = L[Map::at(j + s * (N / R))];
+                for (int s = 0; s < R; ++s) v[b * R + s] = L[Map::shifted(a, s * (N / R))];
+            } else {
+#pragma unroll
+                for (int s = 0; s < R; ++s) v[b * R + s] = L[Map::at(j + s * (N / R))];
+            }
 #pragma unroll
             for (int s = 1; s < R; ++s) v[b * R + s] = cmul(v[b * R + s], w[b * R + s]);
             Dft<R>::run(&v[b * R]);
@@ -127,8 +140,14 @@ template <int LOGN, class Map> struct RegFft {
         for (int b = 0; b < B; ++b) {
             const int j = li + b * T;
             const int o = (j / NS) * (NS * R) + (j & (NS - 1));
+            if constexpr (Map::kSwizzled && NS % 64 == 0) {
+                const int a = Map::at(o);
 #pragma unroll
-            for (int t = 0; t < R; ++t) L[Map::at(o + t * NS)] = v[b * R + t];
+                for (int t = 0; t < R; ++t) L[Map::shifted(a, t * NS)] = v[b * R + t];
+            } else {
+#pragma unroll
+                for (int t = 0; t < R; ++t) L[Map::at(o + t * NS)] = v[b * R + t];
+            }
         }
     }
 
