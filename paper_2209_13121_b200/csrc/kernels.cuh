@@ -234,9 +234,12 @@ __device__ __forceinline__ PixelGeom pixel_geometry(int ix, int iy, int Nx, int 
     if (s2 < 0.0) return g;
     const double root = __dsqrt_rn(s2);
     const double qz = __dsub_rn(root, k);
-    g.r[0] = (float)__ddiv_rn(qx, k);
-    g.r[1] = (float)__ddiv_rn(qy, k);
-    g.r[2] = (float)__ddiv_rn(__dadd_rn(qz, k), k);
+    // r = (q_x, q_y, q_z + k)/k feeds fp32 values only (no decision), so one reciprocal and three
+    // multiplications replace three of the kernel's four double divisions; q_z + k is the root itself
+    const double ik = __drcp_rn(k);
+    g.r[0] = (float)__dmul_rn(qx, ik);
+    g.r[1] = (float)__dmul_rn(qy, ik);
+    g.r[2] = (float)__dmul_rn(root, ik);
     if (Nz == 1) { g.n_nodes = 1; g.node[0] = 0; g.wt[0] = 1.f; return g; }
     const double gz = __ddiv_rn(qz, dqz);
     if (mode == 0) {
