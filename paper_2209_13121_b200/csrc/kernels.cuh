@@ -393,6 +393,93 @@ k_ewald_basis(const EwaldBasisParams q)
     p.img[(((size_t)blockIdx.z * p.Ny + iy) * p.Nx + ix) * EG + sub] = make_float4(axx, ayy, axy, valid ? 1.f : 0.f);
 }
 
+// Ewald projection for SPECTRAL_BASIS on a 2-D model (Nz = 1, A13) with at most EW2D_MAXP packs: the
+// k_z = 0 plane serves every energy, so a thread owns one pixel, gathers and unpacks its basis
+// spectra once (registers) and loops over the batch's energies; per energy only the validity and
+// r-hat (fp64, same operation order as pixel_geometry), the coefficient sum and the projection
+// remain.  Coefficients, k, 1/k and k^4 of the batch sit in shared memory.  Same arithmetic and
+// summation order as k_ewald_basis: identical images.
+constexpr int EW2D_MAXP = 8;
+
+template <int EG>
+__global__ void __launch_bounds__(256)
+k_ewald_basis_2d(const EwaldBasisParams q)
+{
+    const EwaldParams &p = q.g;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int nb = 2 * q.n_pack, ne = p.n_e;
+    double *s_k = reinterpret_cast<double *>(smem_raw);              // [ne] k, then [ne] 1/k
+    double *s_ik = s_k + ne;
+    float2 *s_coef = reinterpret_cast<float2 *>(s_ik + ne);          // [ne][nb]
+    float *s_k4 = reinterpret_cast<float *>(s_coef + (size_t)ne * nb);   // [ne]
+    int *s_kind = reinterpret_cast<int *>(s_k4 + ne);                 // [nb]
+    for (int e = threadIdx.x; e < ne; e += 256) {
+        const double k = p.k[p.e0 + e];
+        s_k[e] = k; s_ik[e] = __drcp_rn(k);
+        const double k2 = k * k;
+        s_k4[e] = (float)(k2 * k2);
+    }
+    for (int i = threadIdx.x; i < ne * nb; i += 256) s_coef[i] = q.coef[(size_t)p.e0 * nb + i];
+    for (int i = threadIdx.x; i < nb; i += 256) s_kind[i] = q.kind[i];
+    __syncthreads();
+    const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int iy = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (ix >= p.Nx || iy >= p.Ny) return;
+    const int mx = ix - p.Nx / 2, my = iy - p.Ny / 2;
+    const int sx = win_slot(p.wx, mx), sy = win_slot(p.wy, my);
+    const int tx = win_slot(p.wx, -mx), ty = win_slot(p.wy, -my);
+    const bool inwin = sx < p.wx.W && sy < p.wy.W && tx < p.wx.W && ty < p.wy.W;
+    const size_t fstride = (size_t)p.wy.W * p.pitch;                 // wz.W == 1
+    const float2 *pq = p.spec + (size_t)sy * p.pitch + sx;
+    const float2 *pm = p.spec + (size_t)ty * p.pitch + tx;
+    float2 F[2 * EW2D_MAXP];
+#pragma unroll
+    for (int pk = 0; pk < EW2D_MAXP; ++pk) {
+        float2 z1 = make_float2(0.f, 0.f), z2 = z1;
+        if (inwin && pk < q.n_pack) { z1 = __ldg(pq + pk * fstride); z2 = __ldg(pm + pk * fstride); }
+        // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
+        F[2 * pk] = make_float2(z1.x + z2.x, z1.y - z2.y);
+        F[2 * pk + 1] = make_float2(z1.y + z2.y, z2.x - z1.x);
+    }
+    const double qx = __dmul_rn((double)mx, p.dqx), qy = __dmul_rn((double)my, p.dqy);
+    const double qx2 = __dmul_rn(qx, qx), qy2 = __dmul_rn(qy, qy);
+    const size_t pix = (size_t)iy * p.Nx + ix, plane = (size_t)p.Ny * p.Nx;
+    for (int e = 0; e < ne; ++e) {
+        const double k = s_k[e];
+        const double s2 = __dsub_rn(__dsub_rn(__dmul_rn(k, k), qx2), qy2);
+        float4 res = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (s2 >= 0.0) {
+            const double ik = s_ik[e];
+            const float r[3] = {(float)__dmul_rn(qx, ik), (float)__dmul_rn(qy, ik), (float)__dmul_rn(__dsqrt_rn(s2), ik)};
+            float2 c[NCHI];
+#pragma unroll
+            for (int f = 0; f < NCHI; ++f) c[f] = make_float2(0.f, 0.f);
+            const float2 *coef = s_coef + (size_t)e * nb;
+            if (inwin) {
+#pragma unroll
+                for (int b = 0; b < 2 * EW2D_MAXP; ++b) {
+                    if (b < nb) {
+                        const int kd = s_kind[b];
+                        const float2 v = cmul(coef[b], F[b]);
+                        if (kd == BK_PHI || kd == BK_W) { c[0] = cadd(c[0], v); c[3] = cadd(c[3], v); }
+                        else if (kd == BK_XX) c[0] = cadd(c[0], v);
+                        else if (kd == BK_YY) c[3] = cadd(c[3], v);
+                        else if (kd == BK_XY) c[1] = cadd(c[1], v);
+                        else if (kd == BK_XZ) c[2] = cadd(c[2], v);
+                        else if (kd == BK_YZ) c[4] = cadd(c[4], v);
+                    }
+                }
+            }
+            const float2 u[3] = {c[0], c[1], c[2]}, v3[3] = {c[1], c[3], c[4]};
+            float sxx, syy, sxy;
+            project_pair(r, u, v3, sxx, syy, sxy);
+            const float w = 1.f * s_k4[e];
+            res = make_float4(fmaf(w, sxx, 0.f), fmaf(w, syy, 0.f), fmaf(w, sxy, 0.f), 1.f);
+        }
+        p.img[((size_t)(e / EG) * plane + pix) * EG + e % EG] = res;
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // Rotate back and average (DESIGN 3-A9/A10).  A thread owns one output pixel and one energy of
 // every energy group (lanes: EG energies x 32/EG pixels, see EwaldParams).  The bilinear cell
