@@ -570,7 +570,7 @@ k_rotate_avg(const RotateParams p)
     const int na = live ? min(p.n_angles, a_begin + per) : 0;
     const int rowq = p.Nx * EG;
     for (int a0 = a_begin; a0 < na; a0 += UA) {
-        int o00[UA], ox[UA], oy[UA];
+        int o00[UA], o10[UA], o01[UA], o11[UA];          // element offsets of the four taps within a group
         float w00[UA], w10[UA], w01[UA], w11[UA], wx[UA], wy[UA], wz[UA];
         bool ok[UA];
 #pragma unroll
@@ -587,22 +587,27 @@ k_rotate_avg(const RotateParams p)
             ok[q] = (a0 + q < na) && !(x0 < 0.0 || y0 < 0.0 || x0 + (double)dx > xmax || y0 + (double)dy > ymax);
             // un-needed neighbours alias a needed one (weight 0, same validity)
             o00[q] = ok[q] ? ((int)y0 * p.Nx + (int)x0) * EG : 0;
-            ox[q] = ok[q] ? dx * EG : 0; oy[q] = ok[q] ? dy * rowq : 0;
+            const int ox = ok[q] ? dx * EG : 0, oy = ok[q] ? dy * rowq : 0;
+            o10[q] = o00[q] + ox; o01[q] = o00[q] + oy; o11[q] = o01[q] + ox;
             const float fa = (float)al, fb = (float)be;
             w00[q] = (1.f - fa) * (1.f - fb); w10[q] = fa * (1.f - fb); w01[q] = (1.f - fa) * fb; w11[q] = fa * fb;
         }
-        for (int j = 0; j < ng; ++j) {
-            if (!((live >> j) & 1u)) continue;
-            const float4 *base = img + (size_t)j * plane;
+        // the groups of this CTA: base pointer, running sums and live bits advance by increments
+        // (no per-group multiplications: address arithmetic was a third of the kernel's instructions)
+        const float4 *base = img;
+        float *ps = s_sum + tid;
+        unsigned int *pc = s_cnt + tid;
+        unsigned int lv = live;
+        for (int j = 0; j < ng; ++j, base += plane, ps += 256, pc += 256, lv >>= 1) {
+            if (!(lv & 1u)) continue;
             float4 t[UA][4];
 #pragma unroll
             for (int q = 0; q < UA; ++q) {
-                const float4 *p00 = base + o00[q];
-                t[q][0] = __ldg(p00); t[q][1] = __ldg(p00 + ox[q]);
-                t[q][2] = __ldg(p00 + oy[q]); t[q][3] = __ldg(p00 + oy[q] + ox[q]);
+                t[q][0] = __ldg(base + o00[q]); t[q][1] = __ldg(base + o10[q]);
+                t[q][2] = __ldg(base + o01[q]); t[q][3] = __ldg(base + o11[q]);
             }
-            float sum = s_sum[j * 256 + tid];
-            unsigned int cnt = s_cnt[j * 256 + tid];
+            float sum = *ps;
+            unsigned int cnt = *pc;
 #pragma unroll
             for (int q = 0; q < UA; ++q) {
                 const float4 t00 = t[q][0], t10 = t[q][1], t01 = t[q][2], t11 = t[q][3];
@@ -613,8 +618,8 @@ k_rotate_avg(const RotateParams p)
                 acc = fmaf(w11[q], wx[q] * t11.x + wy[q] * t11.y + wz[q] * t11.z, acc);
                 if (good) { sum += acc; ++cnt; }
             }
-            s_sum[j * 256 + tid] = sum;
-            s_cnt[j * 256 + tid] = cnt;
+            *ps = sum;
+            *pc = cnt;
         }
     }
     if (AS > 1) __syncthreads();
