@@ -361,13 +361,13 @@ k_ewald_basis(const EwaldBasisParams q)
             for (int j = 0; j < g.n_nodes; ++j) {
                 const int sz = win_slot(p.wz, g.node[j]), tz = win_slot(p.wz, -g.node[j]);
                 const bool ok = inwin && sz < p.wz.W && tz < p.wz.W;
-                const float2 *pq = p.spec + (size_t)sz * plane + (size_t)sy * p.pitch + sx;
+                const float2 *pq = p.spec + (size_t)sz * plane + (size_t)sy * p.pitch + sx;      // advanced pack by pack
                 const float2 *pm = p.spec + (size_t)tz * plane + (size_t)ty * p.pitch + tx;
                 float2 c[NCHI];
 #pragma unroll
                 for (int f = 0; f < NCHI; ++f) c[f] = make_float2(0.f, 0.f);
-                for (int pk = 0; ok && pk < q.n_pack; ++pk) {
-                    const float2 z1 = __ldg(pq + pk * fstride), z2 = __ldg(pm + pk * fstride);
+                for (int pk = 0; ok && pk < q.n_pack; ++pk, pq += fstride, pm += fstride) {
+                    const float2 z1 = __ldg(pq), z2 = __ldg(pm);
                     // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
                     const float2 F[2] = {make_float2(z1.x + z2.x, z1.y - z2.y), make_float2(z1.y + z2.y, z2.x - z1.x)};
 #pragma unroll
