@@ -41,9 +41,9 @@ LIMITER = {"k_xbasis2 (fields + FFT along x)": "HBM stream, instruction-issue li
            "k_ewald_basis (Ewald gather)": "instruction issue + L2 gather latency, not HBM (DESIGN 7.3)",
            "k_rotate_avg (rotate back + average)": "L1 data-pipe wavefronts / latency of the bilinear gathers, not HBM (DESIGN 7.4)"}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (average over the kernel's launches of a step) from the
-# committed ncu --set full capture profiles/r1d_cfg2_ncu_summary.md; ncu flushes the caches before each replay and
+# committed ncu --set full capture profiles/r1e_cfg2_ncu_summary.md; ncu flushes the caches before each replay and
 # part of the writes is still in L2 when a kernel ends, so this can be below the algorithmic bytes
-NCU_TRAFFIC = {("cfg2", "k_xbasis2 (fields + FFT along x)"): 59.2e6, ("cfg2", "k_col2p (FFT along z, then along y)"): 75.5e6,
+NCU_TRAFFIC = {("cfg2", "k_xbasis2 (fields + FFT along x)"): 59.7e6, ("cfg2", "k_col2p (FFT along z, then along y)"): 75.6e6,
                ("cfg2", "k_ewald_basis (Ewald gather)"): 11.6e6, ("cfg2", "k_rotate_avg (rotate back + average)"): 2.4e6}
 
 
@@ -329,6 +329,8 @@ def run_ours(args, rank, world, local_rank):
                            else "resident in HBM"),
         },
         "voxel_angle_evals_per_s": value * w.n_vox,
+        "device_bytes": {"morphology": int(sum(a.nbytes for m in w.materials for a in m if a is not None)) if args.streamed == 0 else 0,
+                         "workspace": int(st["workspace_bytes"])},
         "e2e": {"value": w.n_energy * w.n_angles * world / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms},
         "gpu_launches": int(launches),
