@@ -357,3 +357,25 @@ def test_thin_film_nz63(alg):
     ref, rcnt = oracle_run(w, linear=True)
     out, cnt, _ = _gpu(w, alg)
     print("nz63", compare(out, cnt, ref, rcnt, "nz63"))
+
+
+def test_host_output_across_several_energy_batches():
+    """Pinned-host `out` with more energies than one batch holds (batches of 256): the double-buffered
+    staging area and the copy stream's events are exercised over three batches, twice in a row."""
+    import torch
+    from paper_2209_13121_b200 import binding
+    w = W.tiny(seed=81, nx=16, ny=16, nz=2, n_mat=2, n_energy=600, voxel_nm=3.0, energies=np.linspace(270.0, 340.0, 600))
+    ref, rcnt = oracle_run(w, linear=True)
+    ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    s = torch.cuda.current_stream().cuda_stream
+    ctx.set_morphology_host(w.materials, s)
+    ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald)
+    out = torch.zeros((w.n_energy, w.Ny, w.Nx), dtype=torch.float32).pin_memory()
+    for _ in range(2):
+        out.zero_()
+        ctx.run(out.data_ptr(), s)
+        torch.cuda.synchronize()
+        assert ctx.stats()["energy_batch"] == 256
+        compare(out.numpy(), None, ref, rcnt, "host-io-3-batches")
+    ctx.close()
