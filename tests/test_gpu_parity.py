@@ -379,3 +379,44 @@ def test_host_output_across_several_energy_batches():
         assert ctx.stats()["energy_batch"] == 256
         compare(out.numpy(), None, ref, rcnt, "host-io-3-batches")
     ctx.close()
+
+
+def test_context_reconfiguration_sequence():
+    """One context driven through a sequence of reconfigurations (energies, angles, Ewald mode, algorithm,
+    morphology); every run is compared with the oracle, so cached plans, tables and buffers must follow."""
+    import torch
+    from paper_2209_13121_b200 import binding
+    base = W.tiny(seed=91, nx=32, ny=16, nz=8, n_mat=3, n_energy=12, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR)
+    dev = torch.device("cuda")
+    mats = [tuple(None if a is None else torch.from_numpy(a).to(dev) for a in m) for m in base.materials]
+    ctx = binding.Context(base.Nx, base.Ny, base.Nz, base.n_mat, base.voxel_nm)
+    ctx.set_morphology(mats)
+    s = torch.cuda.current_stream().cuda_stream
+    steps = [
+        dict(idx=range(12), angles=(0.0, 30.0, 150.0), ewald=W.EWALD_TRILINEAR, alg=binding.ALG_AUTO),
+        dict(idx=range(3), angles=(0.0, 30.0, 150.0), ewald=W.EWALD_TRILINEAR, alg=binding.ALG_AUTO),
+        dict(idx=range(3), angles=(10.0, 7.0, 94.0), ewald=W.EWALD_NEAREST, alg=binding.ALG_AUTO),
+        dict(idx=range(2, 11), angles=(10.0, 7.0, 94.0), ewald=W.EWALD_NEAREST, alg=binding.ALG_PER_ENERGY),
+        dict(idx=[5], angles=(45.0, 0.0, 45.0), ewald=W.EWALD_TRILINEAR, alg=binding.ALG_SPECTRAL_BASIS),
+        dict(idx=range(12), angles=(0.0, 90.0, 270.0), ewald=W.EWALD_TRILINEAR, alg=binding.ALG_AUTO),
+    ]
+    for k, st in enumerate(steps):
+        w = base.restrict_energies(list(st["idx"]))
+        w.angles, w.ewald = st["angles"], st["ewald"]
+        if k == 4:      # a different morphology on the same context: isotropic-only
+            iso = [(m[0], None, None, None) for m in base.materials]
+            w = W.Workload("iso", w.Nx, w.Ny, w.Nz, w.voxel_nm, iso, w.energies, w.delta_par, w.beta_par, w.delta_par,
+                           w.beta_par, w.angles, w.ewald)
+            ctx.set_morphology([(m[0], None, None, None) for m in mats])
+        elif k == 5:
+            ctx.set_morphology(mats)
+        ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+        ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald); ctx.set_algorithm(st["alg"])
+        out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32, device=dev)
+        cnt = torch.zeros((w.n_energy, w.Ny, w.Nx), dtype=torch.int32, device=dev)
+        ctx.set_counts_output(cnt.data_ptr())
+        ctx.run(out.data_ptr(), s)
+        torch.cuda.synchronize()
+        ref, rcnt = oracle_run(w)
+        compare(out.cpu().numpy(), cnt.cpu().numpy(), ref, rcnt, f"reconfig step {k}")
+    ctx.close()
