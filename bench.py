@@ -338,7 +338,8 @@ def run_ours(args, rank, world, local_rank):
         "roofline": {"bound": "hbm", "kernel": dom, "stages": dom_stages, "launches_per_step": dom_launches,
                      "share_of_step": ktime[dom] / max(sum(ktime.values()), 1e-12),
                      "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
+                     "frac": achieved / peak, "frac_vs_nominal_8000": achieved / 8000.0,
+                     "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
                      "limiter": LIMITER[dom],
                      "bytes_per_launch": dom_bytes_per_launch, "ms_per_launch": dom_ms_per_launch,
                      "stage_ms_per_step": {k: v / nprof for k, v in stage_ms.items()},
