@@ -420,3 +420,23 @@ def test_context_reconfiguration_sequence():
         ref, rcnt = oracle_run(w)
         compare(out.cpu().numpy(), cnt.cpu().numpy(), ref, rcnt, f"reconfig step {k}")
     ctx.close()
+
+
+def test_streamed_cfg3_reduced():
+    """The CFG3 recipe (3 materials, Voronoi grains, trilinear) at 64 x 64 x 32 through the streamed mode,
+    one material per group, pinned-host output."""
+    import torch
+    from paper_2209_13121_b200 import binding
+    w = W.cfg3(nx=64, ny=64, nz=32, n_energy=4, grain=8.0)
+    ref, rcnt = oracle_run(w, linear=True)
+    pinned = [tuple(None if a is None else torch.from_numpy(a).pin_memory() for a in m) for m in w.materials]
+    ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    ctx.set_morphology_streamed(pinned, 1)
+    ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald)
+    out = torch.zeros((w.n_energy, w.Ny, w.Nx), dtype=torch.float32).pin_memory()
+    s = torch.cuda.current_stream().cuda_stream
+    ctx.run(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    compare(out.numpy(), None, ref, rcnt, "cfg3/64 streamed")
+    ctx.close()
