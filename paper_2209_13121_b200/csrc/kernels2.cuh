@@ -283,14 +283,14 @@ k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
         if (nbuf + (aligned ? 4 : 1) > XB2_PB) flush();
         float ph[R0];
 #pragma unroll
-        for (int s = 0; s < R0; ++s) ph[s] = __ldg(mp.phi[m] + vox0 + (size_t)s * T);
+        for (int s = 0; s < R0; ++s) ph[s] = __ldcs(mp.phi[m] + vox0 + (size_t)s * T);
         if (aligned) {
             float S_[R0], th[R0], ps[R0];
 #pragma unroll
             for (int s = 0; s < R0; ++s) {
-                S_[s] = __ldg(mp.S[m] + vox0 + (size_t)s * T);
-                th[s] = __ldg(mp.theta[m] + vox0 + (size_t)s * T);
-                ps[s] = __ldg(mp.psi[m] + vox0 + (size_t)s * T);
+                S_[s] = __ldcs(mp.S[m] + vox0 + (size_t)s * T);
+                th[s] = __ldcs(mp.theta[m] + vox0 + (size_t)s * T);
+                ps[s] = __ldcs(mp.psi[m] + vox0 + (size_t)s * T);
             }
             float w[R0], dx[R0], dy[R0], dz[R0];
 #pragma unroll
