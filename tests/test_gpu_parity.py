@@ -440,3 +440,26 @@ def test_streamed_cfg3_reduced():
     torch.cuda.synchronize()
     compare(out.numpy(), None, ref, rcnt, "cfg3/64 streamed")
     ctx.close()
+
+
+@pytest.mark.parametrize("shape,n_mat,n_energy", [((128, 128, 128), 2, 10), ((64, 32, 16), 3, 5), ((256, 256, 1), 2, 1)])
+def test_P14_footprint_bound(shape, n_mat, n_energy):
+    """Device scratch against the memory model (Table 1 counts (4c + 6) N + 2 NxNy reals for Alg. 1): the
+    SPECTRAL_BASIS workspace is at most three pruned copies of the n_pack complex basis cubes plus the interleaved
+    images, i.e. <= 3 * 8 * n_pack * N + 16 * NxNy * (n_energy rounded up to a group of 8) bytes, and it does not
+    grow when the same run is repeated."""
+    from paper_2209_13121_b200 import binding
+    nx, ny, nz = shape
+    w = W.tiny(seed=5, nx=nx, ny=ny, nz=nz, n_mat=n_mat, n_energy=n_energy, voxel_nm=2.0)
+    out, ctx = binding.simulate(w, algorithm=binding.ALG_SPECTRAL_BASIS)
+    n_fields = sum(7 if m[1] is not None else 1 for m in w.materials)
+    n_pack = (n_fields + 1) // 2
+    N = nx * ny * nz
+    pitch_factor = max(1.0, 32.0 / nx)                       # rows are padded to 32 complex values
+    bound = 3 * 8 * n_pack * N * pitch_factor + 16 * nx * ny * ((n_energy + 7) // 8 * 8) + 4096
+    ws = ctx.stats()["workspace_bytes"]
+    assert 0 < ws <= bound, (ws, bound)
+    import torch
+    ctx.run(out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert ctx.stats()["workspace_bytes"] == ws
