@@ -1,7 +1,8 @@
 // kernels.cuh -- the sm_100a kernels of the CyRSoXS hot path.
 //   k_xpass_chi   polarization (Eq. 2-5) fused with the FFT along x, pruned store
 //   (k_xbasis2, k_col2p, k_col2: the SPECTRAL_BASIS x pass and the column passes, kernels2.cuh)
-//   k_ewald_chi   Ewald gather (Eq. 8) + (I - r r^T) + |.|^2 (Eq. 7) -> (I_xx, I_yy, I_xy, valid)
+//   k_ewald_chi, k_ewald_basis, k_ewald_basis_2d
+//                 Ewald gather (Eq. 8) + (I - r r^T) + |.|^2 (Eq. 7) -> (I_xx, I_yy, I_xy, valid)
 //   k_rotate_avg  rotate back by -zeta (bilinear), accumulate over angles, divide by counts
 // Geometry decisions use IEEE double with explicitly rounded operations (__dmul_rn ...), the
 // same sequence DESIGN.md 3-A11 writes out, so validity/cell decisions do not depend on FMA
