@@ -56,15 +56,16 @@ typedef enum {
  *                   transformed, and projected.
  *   SPECTRAL_BASIS  p is also linear in the optical constants: the energy-independent real
  *                   fields phi, phi S, phi S d_i d_j are transformed once per run and every
- *                   energy only combines their spectra on its Ewald shell (DESIGN 7.2).
- *   AUTO            picks whichever moves fewer bytes for the configured run. */
+ *                   energy only combines their spectra on its Ewald shell (DESIGN 7.0).
+ *   AUTO            SPECTRAL_BASIS unless the basis needs more than 10 complex transforms per
+ *                   energy of the run (n_pack > 10 n_energy: one energy, many aligned materials). */
 typedef enum {
     CYRSOXS_ALG_AUTO = 0,
     CYRSOXS_ALG_PER_ENERGY = 1,
     CYRSOXS_ALG_SPECTRAL_BASIS = 2
 } cyrsoxs_algorithm;
 
-/* Stage ids for cyrsoxs_stage_times / cyrsoxs_debug_fetch. */
+/* Stage ids of cyrsoxs_stats (stage_launches, stage_bytes, stage_ms). */
 typedef enum {
     CYRSOXS_STAGE_XPASS = 0,   /* polarization (or basis fields) fused with the FFT along x  */
     CYRSOXS_STAGE_ZPASS = 1,   /* FFT along z, pruned to the k_z planes the Ewald shells touch */
