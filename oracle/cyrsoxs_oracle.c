@@ -260,9 +260,10 @@ void orc_dft3_naive(int Nx, int Ny, int Nz, const cplx *in, cplx *out)
             }
 }
 
-/* Direct evaluation of p~ at a list of bins, straight from the morphology
- * (O2 then the sum of Eq. 6 for those bins only): O(n_vox * n_bins).  Used to
- * spot-check full-size runs where a whole double-precision FFT is too big.
+/* Direct evaluation of p~ at a list of bins: the sum of Eq. 6 written out for those
+ * bins only, over the polarization field that orc_polarization (O2, the single statement of
+ * Eq. 2-5 in this file) produces slab by slab: O(n_vox * n_bins).  Used to spot-check sizes
+ * where a whole double-precision FFT is too big.
  * bins: n_bins x 3 ints (kx, ky, kz), any integers (taken mod N).
  * out:  n_bins x 3 complex (p~x, p~y, p~z). */
 void orc_polarization_dft_bins(int Nx, int Ny, int Nz, int n_mat,
@@ -272,60 +273,40 @@ void orc_polarization_dft_bins(int Nx, int Ny, int Nz, int n_mat,
                                double ex, double ey, double ez,
                                int n_bins, const int *bins, cplx *out)
 {
-    const double inv4pi = 1.0 / (4.0 * ORC_PI);
     const int64_t n_vox = (int64_t)Nx * Ny * Nz;
-    int nthr = orc_num_threads();
-    cplx *part = (cplx *)calloc((size_t)nthr * n_bins * 3, sizeof(cplx));
-#pragma omp parallel
-    {
-#ifdef _OPENMP
-        int t = omp_get_thread_num();
-#else
-        int t = 0;
-#endif
-        cplx *acc = part + (size_t)t * n_bins * 3;
-#pragma omp for schedule(static)
-        for (int64_t i = 0; i < n_vox; ++i) {
-            int x = (int)(i % Nx), y = (int)((i / Nx) % Ny), z = (int)(i / ((int64_t)Nx * Ny));
+    const int64_t chunk = n_vox < ((int64_t)1 << 22) ? n_vox : ((int64_t)1 << 22);
+    cplx *px = (cplx *)malloc(sizeof(cplx) * (size_t)chunk), *py = (cplx *)malloc(sizeof(cplx) * (size_t)chunk),
+         *pz = (cplx *)malloc(sizeof(cplx) * (size_t)chunk);
+    const float **tab = (const float **)malloc(sizeof(float *) * 4 * (size_t)n_mat);
+    for (int q = 0; q < 3 * n_bins; ++q) out[q] = 0.0;
+    for (int64_t i0 = 0; i0 < n_vox; i0 += chunk) {
+        const int64_t n = n_vox - i0 < chunk ? n_vox - i0 : chunk;
+        for (int m = 0; m < n_mat; ++m) {
+            tab[m] = phi[m] + i0;
+            tab[n_mat + m] = S[m] ? S[m] + i0 : NULL;
+            tab[2 * n_mat + m] = theta[m] ? theta[m] + i0 : NULL;
+            tab[3 * n_mat + m] = psi[m] ? psi[m] + i0 : NULL;
+        }
+        orc_polarization(n, n_mat, tab, tab + n_mat, tab + 2 * n_mat, tab + 3 * n_mat, a, b, c, ex, ey, ez, px, py, pz);
+#pragma omp parallel for schedule(static)
+        for (int q = 0; q < n_bins; ++q) {
+            int64_t kx = ((bins[3 * q] % Nx) + Nx) % Nx;
+            int64_t ky = ((bins[3 * q + 1] % Ny) + Ny) % Ny;
+            int64_t kz = ((bins[3 * q + 2] % Nz) + Nz) % Nz;
             cplx sx = 0.0, sy = 0.0, sz = 0.0;
-            for (int m = 0; m < n_mat; ++m) {
-                double f = (double)phi[m][i];
-                double s = S[m] ? (double)S[m][i] : 0.0;
-                cplx am = a[2 * m] + I * a[2 * m + 1];
-                cplx bm = b[2 * m] + I * b[2 * m + 1];
-                cplx cm = c[2 * m] + I * c[2 * m + 1];
-                cplx iso = (1.0 - s) * cm;
-                cplx tx = iso * ex, ty = iso * ey, tz = iso * ez;
-                if (s != 0.0) {
-                    double th = theta[m] ? (double)theta[m][i] : 0.0;
-                    double ps = psi[m] ? (double)psi[m][i] : 0.0;
-                    double dx = cos(ps) * sin(th), dy = sin(ps) * sin(th), dz = cos(th);
-                    double de = dx * ex + dy * ey + dz * ez;
-                    tx += s * (am * ex + bm * (de * dx));
-                    ty += s * (am * ey + bm * (de * dy));
-                    tz += s * (am * ez + bm * (de * dz));
-                }
-                sx += f * tx; sy += f * ty; sz += f * tz;
-            }
-            sx *= inv4pi; sy *= inv4pi; sz *= inv4pi;
-            for (int q = 0; q < n_bins; ++q) {
-                int64_t kx = ((bins[3 * q] % Nx) + Nx) % Nx;
-                int64_t ky = ((bins[3 * q + 1] % Ny) + Ny) % Ny;
-                int64_t kz = ((bins[3 * q + 2] % Nz) + Nz) % Nz;
+            for (int64_t l = 0; l < n; ++l) {
+                const int64_t i = i0 + l;
+                int x = (int)(i % Nx), y = (int)((i / Nx) % Ny), z = (int)(i / ((int64_t)Nx * Ny));
                 double ph = (double)(kx * x % Nx) / Nx + (double)(ky * y % Ny) / Ny
                           + (double)(kz * z % Nz) / Nz;
                 double ang = -2.0 * ORC_PI * ph;
                 cplx w = cos(ang) + I * sin(ang);
-                acc[3 * q] += sx * w; acc[3 * q + 1] += sy * w; acc[3 * q + 2] += sz * w;
+                sx += px[l] * w; sy += py[l] * w; sz += pz[l] * w;
             }
+            out[3 * q] += sx; out[3 * q + 1] += sy; out[3 * q + 2] += sz;
         }
     }
-    for (int q = 0; q < 3 * n_bins; ++q) {
-        cplx s = 0.0;
-        for (int t = 0; t < nthr; ++t) s += part[(size_t)t * n_bins * 3 + q];
-        out[q] = s;
-    }
-    free(part);
+    free(px); free(py); free(pz); free(tab);
 }
 
 /* ------------------------------------------------------------------ O4 -- */

@@ -110,6 +110,9 @@ def test_P1_full_pipeline_with_bruteforce_dft():
 
 
 def test_dft_bins_match_fft():
+    """Pins only the bin SUMMATION of polarization_dft_bins (Eq. 6 written out for single bins) against the
+    FFT of the same field; the polarization itself comes from the one statement orc_polarization on both sides
+    and is pinned elsewhere (P2, P3, P9, P10, R2a)."""
     w = W.tiny(seed=6, nx=16, ny=8, nz=4, n_mat=2, n_energy=1)
     a, b, c = _consts(w)
     e = (0.3, -0.8, 0.0)
@@ -563,3 +566,280 @@ def test_A14_any_Nz_definition_dft_along_z():
     a, ca = _run(w)
     b, cb = _run(w, linear=True)
     assert np.array_equal(ca, cb) and np.allclose(a, b, rtol=1e-11, atol=1e-14 * a.max())
+
+
+# ================================================================ round-2 pins
+# Each of these ties one decision of the oracle, that no earlier pin reached, to a closed form written
+# out here from the paper's equations (none calls the oracle for its expected value).
+
+def _aligned_film(phi1, theta, psi, S, consts_al, consts_iso, voxel, E, angles, ewald=W.EWALD_NEAREST):
+    """Material 1 aligned with a constant director (theta, psi) and alignment S, material 2 = 1 - phi1 isotropic.
+    consts_al = (delta_par, beta_par, delta_perp, beta_perp), consts_iso = (delta, beta)."""
+    phi1 = np.ascontiguousarray(phi1, np.float32)
+    full = lambda v: np.full(phi1.shape, v, np.float32)
+    mats = [(phi1, full(S), full(theta), full(psi)), (np.ascontiguousarray(1.0 - phi1, dtype=np.float32), None, None, None)]
+    nz, ny, nx = phi1.shape
+    f = lambda a, b: np.array([[a, b]], np.float32)
+    dpa, bpa, dpe, bpe = consts_al
+    di, bi = consts_iso
+    return W.Workload("aligned", nx, ny, nz, voxel, mats, np.array([E]), f(dpa, di), f(bpa, bi), f(dpe, di), f(bpe, bi),
+                      angles, ewald)
+
+
+def _n(delta, beta):
+    """n = 1 - delta + i beta with the float32-rounded constants the oracle receives (north_star)."""
+    return 1 - float(np.float32(delta)) + 1j * float(np.float32(beta))
+
+
+@pytest.mark.parametrize("theta_deg,psi_deg,zeta", [(35.0, 20.0, 0.0), (120.0, -50.0, 0.0), (60.0, 75.0, 90.0)])
+def test_R2a_uniform_director_plane_wave_film(theta_deg, psi_deg, zeta):
+    """Eq. 2-5 and Eq. 7-8 on a film whose only structure is one Fourier mode:
+    material 1 fully aligned (S = 1) with a constant director out of the film plane (theta != 90 deg),
+    phi1 = 1/2 + 1/2 cos(2 pi a x / Nx), material 2 = 1 - phi1 isotropic, Nz = 1, one angle.
+    For q != 0:  p~(q) = phi~1(q) (chi_al - chi_iso) e,  chi_al = (a I + b d d^T)/4pi with a = n_perp^2 - 1,
+    b = n_par^2 - n_perp^2,  chi_iso = (n_iso^2 - 1) I/4pi,  and the pixel (+-a, 0) holds
+        I = k^4 |phi~1|^2 || (I - r r^T)(chi_al - chi_iso) e ||^2,  r = (q_x, 0, sqrt(k^2 - q_x^2))/k.
+    The z component of p (b (d.e) d_z) enters through r_z: this value depends on p_z, on which of a / c
+    multiplies the aligned part, and on the (d.e) d term.  zeta = 0 and 90 keep the rotate step a pixel
+    permutation, so the expected value sits at an exact pixel."""
+    nx = ny = 64; a_ = 6; voxel = 2.0; E = 285.0          # dq = 0.049: r_x = 0.204, r_z = 0.979
+    x = np.arange(nx)
+    phi = ((0.5 + 0.5 * np.cos(2 * PI * a_ * x / nx))[None, None, :] * np.ones((1, ny, 1))).astype(np.float32)
+    th, ps = np.deg2rad(theta_deg), np.deg2rad(psi_deg)
+    al, iso = (2.4e-3, 1.1e-3, 0.6e-3, 0.3e-3), (1.3e-3, 0.7e-3)
+    w = _aligned_film(phi, th, ps, 1.0, al, iso, voxel, E, (zeta, 0.0, zeta))
+    out, cnt = _run(w)
+    # --- the closed form, written from the equations
+    k = 2 * PI * E / 1239.84197
+    npar, nperp, niso_m = _n(al[0], al[1]), _n(al[2], al[3]), _n(*iso)
+    thf, psf = float(np.float32(th)), float(np.float32(ps))          # the float32 angles the oracle receives
+    d = np.array([np.cos(psf) * np.sin(thf), np.sin(psf) * np.sin(thf), np.cos(thf)])
+    chi_al = ((nperp ** 2 - 1) * np.eye(3) + (npar ** 2 - nperp ** 2) * np.outer(d, d)) / (4 * PI)
+    chi_iso = (niso_m ** 2 - 1) * np.eye(3) / (4 * PI)
+    e = np.array([np.cos(np.deg2rad(zeta)), np.sin(np.deg2rad(zeta)), 0.0])
+    if zeta == 90.0:
+        e = np.array([0.0, 1.0, 0.0])
+    amp = np.fft.fft2(phi[0].astype(np.float64))[0, a_]               # library FFT of the very same float32 array
+    assert abs(abs(amp) - nx * ny / 4) < 1e-3 * nx * ny
+    dq = 2 * PI / (nx * voxel)
+    c = nx // 2
+    for sgn in (+1, -1):
+        qx = sgn * a_ * dq
+        r = np.array([qx, 0.0, np.sqrt(k * k - qx * qx)]) / k
+        pt = abs(amp) * (chi_al - chi_iso) @ e
+        wv = pt - r * (r @ pt)
+        expect = k ** 4 * np.vdot(wv, wv).real
+        # material-frame pixel (sgn a, 0); the output is the image turned by -zeta: (u, v) -> R(-zeta)(u, v)
+        u, v = (sgn * a_, 0) if zeta == 0.0 else (0, -sgn * a_)
+        got = out[0, c + v, c + u]
+        assert abs(got - expect) <= 2e-7 * expect, (sgn, got, expect)     # float32 rounding of 1 - phi1
+    # what the mutants would give, to show the case separates them: p_z dropped / c in place of a
+    qx = a_ * dq; r = np.array([qx, 0.0, np.sqrt(k * k - qx * qx)]) / k
+    pt = abs(amp) * (chi_al - chi_iso) @ e
+    for bad in (pt * np.array([1, 1, 0]),
+                abs(amp) * ((((niso_m * 0 + ((npar + 2 * nperp) / 3) ** 2 - 1) * np.eye(3)
+                              + (npar ** 2 - nperp ** 2) * np.outer(d, d)) / (4 * PI) - chi_iso) @ e)):
+        wb = bad - r * (r @ bad)
+        good = pt - r * (r @ pt)
+        assert abs(np.vdot(wb, wb).real / np.vdot(good, good).real - 1) > 1e-3
+
+
+def test_R2a_director_along_x_uniform_film():
+    """One fully aligned material filling the film, d = x (theta = 90 deg, psi = 0):  at q = 0, r = z and
+    I(0) = k^4 N^2 |n_par^2 - 1|^2 / 16 pi^2 for e = x (zeta = 0), |n_perp^2 - 1|^2 for e = y (zeta = 90)."""
+    n, voxel, E = 32, 5.0, 285.0
+    dpa, bpa, dpe, bpe = 2.4e-3, 1.1e-3, 0.6e-3, 0.3e-3
+    phi = np.ones((1, n, n), np.float32)
+    mats = [(phi, phi.copy(), np.full_like(phi, np.float32(PI / 2)), np.zeros_like(phi))]
+    f = lambda v: np.array([[v]], np.float32)
+    k = 2 * PI * E / 1239.84197
+    thf = float(np.float32(PI / 2))                   # float32(pi/2): d_z = cos(thf) = -4.4e-8, below the tolerance
+    assert abs(np.cos(thf)) < 1e-7
+    for zeta, nn in ((0.0, _n(dpa, bpa)), (90.0, _n(dpe, bpe))):
+        out, cnt = oracle.run(mats, voxel, [E], f(dpa), f(bpa), f(dpe), f(bpe), (zeta, 0.0, zeta), W.EWALD_NEAREST)
+        I0 = k ** 4 * (n * n) ** 2 * abs(nn ** 2 - 1) ** 2 / (16 * PI ** 2)
+        assert abs(out[0, n // 2, n // 2] - I0) <= 1e-6 * I0
+        off = out[0].copy(); off[n // 2, n // 2] = 0
+        assert off.max() <= 1e-12 * I0
+
+
+def test_R2b_nearest_takes_floor_of_g_plus_half():
+    """P13 with a = 11: g = q_z/dq_z = -1.236, so floor(g) = -2 but the nearest node is floor(g + 1/2) = -1
+    (DESIGN 3-A8).  A plane wave at k_z = -1 must light pixel (+a, 0) with weight 1 in NEAREST mode and
+    weight t = g - floor(g) in TRILINEAR mode; a wave at k_z = -2 must be dark in NEAREST mode."""
+    nx = ny = 64; nz = 16; a_ = 11
+    z, y, x = np.mgrid[0:nz, 0:ny, 0:nx]
+    d1, b1, d2, b2 = 2e-3, 1e-3, 5e-4, 2e-4
+    E, voxel = 285.0, 1.0
+    k = 2 * PI * E / 1239.84197
+    dqx = 2 * PI / (nx * voxel); dqz = 2 * PI / (nz * voxel)
+    qx = a_ * dqx
+    g = (np.sqrt(k * k - qx * qx) - k) / dqz
+    assert -1.5 < g < -1.0                            # nearest node -1, lower node -2
+    t = g + 2.0
+    n1, n2 = _n(d1, b1), _n(d2, b2)
+    c = nx // 2
+    for m_, near_w, tri_w in ((1, 1.0, t), (2, 0.0, 1.0 - t)):
+        phi = (0.5 + 0.5 * np.cos(2 * PI * (a_ * x / nx - m_ * z / nz))).astype(np.float32)
+        amp = abs(np.fft.fftn(phi.astype(np.float64))[(-m_) % nz, 0, a_])
+        X = k ** 4 * abs(n1 ** 2 - n2 ** 2) ** 2 / (16 * PI ** 2) * amp ** 2 * (1 - (qx / k) ** 2)
+        for mode, wt in ((W.EWALD_NEAREST, near_w), (W.EWALD_TRILINEAR, tri_w)):
+            w = _iso_film(phi, d1, b1, d2, b2, voxel, E, (0, 0, 0), ewald=mode)
+            out, cnt = _run(w)
+            assert abs(out[0, c, c + a_] - wt * X) <= 1e-7 * X, (m_, mode, out[0, c, c + a_] / X, wt)
+
+
+def test_R2c_node_range_boundary():
+    """Eq. 8 + DESIGN 3-A8/A14: a pixel is invalid if its (lower / nearest) node lies below -Nz/2; the
+    node -Nz/2 itself is valid.  64 x 64 x 8 at 2.75 nm, 285 eV: k/dq = 40.457 px ((k/dq)^2 = 1636.75),
+    g_min = -5.06, -Nz/2 = -4.  Pixels (m_x, m_y), |m|^2 in brackets, g = (sqrt(k^2 - |m|^2 dq^2) - k)/dq_z
+    worked out by hand (and re-derived below):
+      (30, -24) [1476]  g = -3.472: TRILINEAR nodes (-4, -3) valid;           NEAREST n = -3 valid
+      (31, -24) [1537]  g = -3.809: TRILINEAR lower node -4 = -Nz/2 -> valid; NEAREST n = -4 = -Nz/2 -> valid
+      (28, -28) [1568]  g = -4.021: TRILINEAR lower node -5 -> INVALID;       NEAREST n = -4 -> valid
+      (29, -28) [1625]  g = -4.629: TRILINEAR -5 -> INVALID;                  NEAREST n = -5 -> INVALID
+      (31, -26) [1637]  off the sphere (1637 > 1636.75) -> invalid in both modes."""
+    nx = ny = 64; nz = 8; voxel = 2.75; E = 285.0
+    k = 2 * PI * E / 1239.84197
+    dq = 2 * PI / (nx * voxel); dqz = 2 * PI / (nz * voxel)
+    c = nx // 2
+    gv = lambda mx, my: (np.sqrt(k * k - (mx * mx + my * my) * dq * dq) - k) / dqz
+    for (mx, my), gg in (((30, -24), -3.472), ((31, -24), -3.809), ((28, -28), -4.021), ((29, -28), -4.629)):
+        assert abs(gv(mx, my) - gg) < 1e-3
+    assert 1636 < (k / dq) ** 2 < 1637
+    tri = oracle.ewald_nodes(nx, ny, nz, voxel, k, W.EWALD_TRILINEAR)
+    nea = oracle.ewald_nodes(nx, ny, nz, voxel, k, W.EWALD_NEAREST)
+    px = lambda t, mx, my: (int(t[0][c + my, c + mx]), int(t[1][c + my, c + mx]), bool(t[4][c + my, c + mx]))
+    BAD = -2 ** 31
+    for sx, sy in ((1, 1), (-1, 1), (1, -1), (-1, -1)):       # the rule depends on |q| only; m = -32 does not occur here
+        assert px(tri, sx * 30, sy * 24) == (-4, -3, True) and px(nea, sx * 30, sy * 24) == (-3, BAD, True)
+        assert px(tri, sx * 31, sy * 24) == (-4, -3, True) and px(nea, sx * 31, sy * 24) == (-4, BAD, True)
+        assert px(tri, sx * 28, sy * 28) == (BAD, BAD, False) and px(nea, sx * 28, sy * 28) == (-4, BAD, True)
+        assert px(tri, sx * 29, sy * 28) == (BAD, BAD, False) and px(nea, sx * 29, sy * 28) == (BAD, BAD, False)
+        assert px(tri, sx * 31, sy * 26) == (BAD, BAD, False) and px(nea, sx * 31, sy * 26) == (BAD, BAD, False)
+    # the weights at a boundary pixel: t = g - floor(g) on the upper node
+    t = gv(31, -24) + 4.0
+    assert abs(tri[3][c - 24, c + 31] - t) < 1e-12 and abs(tri[2][c - 24, c + 31] - (1 - t)) < 1e-12
+    # the whole detector against the rule, with every class present and no pixel within 1e-9 of a decision
+    m = np.arange(nx) - c
+    r2 = (m[None, :] ** 2 + m[:, None] ** 2).astype(np.float64)
+    on = r2 * dq * dq <= k * k
+    g = np.where(on, (np.sqrt(np.maximum(k * k - r2 * dq * dq, 0.0)) - k) / dqz, np.nan)
+    assert np.nanmin(np.abs(g - np.round(g))[r2 > 0]) > 1e-9 and np.nanmin(np.abs(g + 0.5 - np.round(g + 0.5))) > 1e-9
+    lo = np.floor(g); nr = np.floor(g + 0.5)
+    exp_tri = on & (lo >= -4); exp_nea = on & (nr >= -4)
+    for cls in (on & (lo == -5), on & (lo == -4), on & (nr == -5), on & (nr == -4), ~on):
+        assert cls.any()
+    assert (tri[4].astype(bool) == exp_tri).all() and (nea[4].astype(bool) == exp_nea).all()
+    assert (tri[0][exp_tri] == lo[exp_tri]).all() and (nea[0][exp_nea] == nr[exp_nea]).all()
+
+
+def _rotate_count_numpy(valid, zeta_deg, rho=1.0):
+    """Independent statement of DESIGN 3-A9/A10 for the counts: output pixel q' samples the source position
+    R(+zeta) q' (physical q; y pixels are rho x-pixels tall); it counts iff every neighbour with non-zero
+    bilinear weight is inside the image and valid.  Plain Python loops; returns (count 0/1, weights)."""
+    ny, nx = valid.shape
+    z = np.deg2rad(zeta_deg)
+    C, S = np.cos(z), np.sin(z)
+    cnt = np.zeros((ny, nx), np.uint32)
+    for iy in range(ny):
+        for ix in range(nx):
+            u, v = ix - nx // 2, (iy - ny // 2) * rho            # in units of dq_x
+            su, sv = C * u - S * v, S * u + C * v                 # source, same units
+            fx, fy = su + nx // 2, sv / rho + ny // 2
+            x0, y0 = int(np.floor(fx)), int(np.floor(fy))
+            ax, ay = fx - x0, fy - y0
+            need = [(x0 + jx, y0 + jy) for jx, wx in ((0, 1 - ax), (1, ax)) for jy, wy in ((0, 1 - ay), (1, ay)) if wx * wy > 0]
+            if all(0 <= X < nx and 0 <= Y < ny and valid[Y, X] for X, Y in need):
+                cnt[iy, ix] = 1
+    return cnt
+
+
+def test_R2d_rotate_with_the_ewald_disk_cutting_the_detector():
+    """O5 (DESIGN 3-A9/A10) where part of the detector is off the Ewald sphere (32 x 32, 0.4 nm voxels:
+    k/dq = 2.94 px at 285 eV -- and a second, larger disk): a sample counts only if EVERY needed neighbour is
+    valid.  Pins: (i) the counts against an independent NumPy statement of that rule; (ii) for an image that is
+    constant on the valid set the average must be exactly that constant wherever cnt > 0 (the weights of a
+    counted sample sum to 1), which fails if invalid neighbours were skipped instead of vetoing the sample."""
+    n = 32
+    m = np.arange(n) - n // 2
+    r2 = m[None, :] ** 2 + m[:, None] ** 2
+    for radius in (2.94, 9.3):
+        valid = (r2 <= radius * radius).astype(np.uint8)
+        img = np.where(valid > 0, 7.25, 1e9)                  # junk outside: must never be read into a counted sample
+        for zeta in (30.0, 77.0):
+            acc = np.zeros((n, n)); cnt = np.zeros((n, n), np.uint32)
+            oracle.rotate_accumulate(img, valid, zeta, acc, cnt)
+            exp = _rotate_count_numpy(valid.astype(bool), zeta)
+            assert (cnt == exp).all()
+            assert 0 < exp.sum() < valid.sum()                 # the rim of the disk loses samples
+            assert np.abs(acc[cnt > 0] - 7.25).max() < 1e-12
+            assert (acc[cnt == 0] == 0).all()
+            # certain cases from geometry alone: well inside the disk every neighbour is valid, well outside none is
+            rr = np.sqrt(r2)
+            assert (cnt[rr <= radius - 1.4143] == 1).all() and (cnt[rr >= radius + 1.4143] == 0).all()
+    # the whole pipeline on such a detector: counts of a multi-angle run = sum of the per-angle rule
+    w = W.tiny(seed=10, nx=32, ny=32, nz=1, n_mat=2, n_energy=1, voxel_nm=0.4, ewald=W.EWALD_NEAREST, angles=(0.0, 30.0, 150.0))
+    out, cnt = _run(w)
+    k = 2 * PI * w.energies[0] / 1239.84197
+    dq = 2 * PI / (n * 0.4)
+    valid = r2 * dq * dq <= k * k
+    exp = sum(_rotate_count_numpy(valid, 30.0 * i) for i in range(6))
+    assert (cnt[0] == exp).all() and 0 < (exp > 0).sum() < n * n
+
+
+def test_R2e_rotation_is_in_physical_q_on_a_non_square_detector():
+    """DESIGN 3-A9: the image rotation acts on physical q.  64 x 32 voxels (rho = Nx/Ny = 2, dq_y = 2 dq_x):
+    stripes along x with m = 8 periods put the first orders at q = +-(8 dq_x, 0); at zeta = 30 deg they must
+    appear at q' = R(-zeta) q = 8 dq_x (cos, -sin) = (6.93 dq_x, -2.0 dq_y): pixel offsets +-(7, -2).
+    Rotating pixel indices instead (rho dropped) would give (7, -4)."""
+    nx, ny, m_ = 64, 32, 8
+    x = np.arange(nx)
+    phi = (0.5 + 0.5 * np.cos(2 * PI * m_ * x / nx))[None, None, :] * np.ones((1, ny, 1))
+    w = _iso_film(phi.astype(np.float32), 2e-3, 1e-3, 5e-4, 2e-4, 5.0, 285.0, (30.0, 0.0, 30.0))
+    out, cnt = _run(w)
+    img = out[0].copy(); cy, cx = ny // 2, nx // 2
+    img[cy - 1:cy + 2, cx - 2:cx + 3] = 0                     # the q = 0 peak and its bilinear leakage
+    iy, ix = np.unravel_index(np.argmax(img), img.shape)
+    assert (ix - cx, iy - cy) in [(7, -2), (-7, 2)]
+    assert img[cy - 4, cx + 7] < 1e-3 * img.max() and img[cy + 4, cx - 7] < 1e-3 * img.max()
+    # counts on the non-square detector against the independent statement (rho = 2)
+    exp = _rotate_count_numpy(np.ones((ny, nx), bool), 30.0, rho=2.0)
+    assert (cnt[0] == exp).all() and 0 < exp.sum() < nx * ny
+    # zeta = 90 deg: q' = (u dq_x, v dq_y) samples q = (-v dq_y, u dq_x), i.e. source pixel (cx - 2 v, cy + u/2):
+    # the +-first orders of the same grating land at q' = (0, -+8 dq_x) = (0, -+4 dq_y): pixels (0, -+4)
+    w = _iso_film(phi.astype(np.float32), 2e-3, 1e-3, 5e-4, 2e-4, 5.0, 285.0, (90.0, 0.0, 90.0))
+    out, cnt = _run(w)
+    img = out[0].copy(); img[cy - 1:cy + 2, cx - 2:cx + 3] = 0
+    iy, ix = np.unravel_index(np.argmax(img), img.shape)
+    assert (ix - cx, abs(iy - cy)) == (0, 4)
+
+
+def test_R2f_polarization_from_the_rotated_index_tensor():
+    """Eq. 1-5 in their tensor form, per voxel, for ANY field direction (e_z != 0 included):
+    the uniaxial index tensor N = diag(n_perp, n_perp, n_par) (extraordinary axis along z before rotation)
+    is rotated by R = Rz(psi) Ry(theta) (which carries z onto d = (cos psi sin theta, sin psi sin theta, cos theta)),
+    N_rot = R N R^T, and p = phi [ S (N_rot N_rot - I) + (1 - S)(n_iso^2 - 1) I ] e / 4 pi.  The oracle uses the
+    director shortcut a e + b (d.e) d; this test builds the matrices."""
+    rng = np.random.default_rng(17)
+    nv = 24
+    phi = rng.uniform(0.1, 1.0, (1, 1, nv)).astype(np.float32)
+    S = rng.uniform(0.0, 1.0, (1, 1, nv)).astype(np.float32)
+    th = rng.uniform(0.0, PI, (1, 1, nv)).astype(np.float32)
+    ps = rng.uniform(-PI, 2 * PI, (1, 1, nv)).astype(np.float32)
+    dpa, bpa, dpe, bpe = 2.4e-3, 1.1e-3, 0.6e-3, 0.3e-3
+    a, b, c = oracle.coefficients([dpa], [bpa], [dpe], [bpe])
+    npar, nperp = _n(dpa, bpa), _n(dpe, bpe)
+    niso = (npar + 2 * nperp) / 3
+    for e in ((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0), (0.3, -0.5, 0.81)):
+        p = oracle.polarization([(phi, S, th, ps)], a, b, c, e)          # [3][1][1][nv]
+        for i in range(nv):
+            t, q = float(th[0, 0, i]), float(ps[0, 0, i])
+            Ry = np.array([[np.cos(t), 0, np.sin(t)], [0, 1, 0], [-np.sin(t), 0, np.cos(t)]])
+            Rz = np.array([[np.cos(q), -np.sin(q), 0], [np.sin(q), np.cos(q), 0], [0, 0, 1]])
+            R = Rz @ Ry
+            Nrot = R @ np.diag([nperp, nperp, npar]) @ R.T
+            s_, f_ = float(S[0, 0, i]), float(phi[0, 0, i])
+            chi = f_ * (s_ * (Nrot @ Nrot - np.eye(3)) + (1 - s_) * (niso ** 2 - 1) * np.eye(3)) / (4 * PI)
+            ref = chi @ np.array(e)
+            assert np.abs(p[:, 0, 0, i] - ref).max() <= 1e-14, (e, i)
