@@ -35,7 +35,9 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB.with_suffix(f".{os.getpid()}.tmp")
-    cmd = [nvcc, *NVCC_FLAGS, "-o", str(tmp), *map(str, SOURCES)]
+    # CYRSOXS_NVCC_EXTRA: extra flags for experiments (e.g. -DCYRSOXS_TUNING); the shipped library is built without
+    extra = os.environ.get("CYRSOXS_NVCC_EXTRA", "").split()
+    cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", str(tmp), *map(str, SOURCES)]
     res = subprocess.run(cmd, capture_output=True, text=True)
     (PKG / "build.log").write_text(" ".join(cmd) + "\n" + res.stdout + res.stderr)
     if res.returncode != 0:

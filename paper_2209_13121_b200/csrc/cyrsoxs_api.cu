@@ -54,11 +54,14 @@ struct cyrsoxs_ctx {
     int nE = 0;
     std::vector<double> energies, k;
     std::vector<float> coef;           // [nE][n_mat][6]: Cc, Ca, Cb (complex) / 4 pi
+    std::vector<float> reach2;         // [nE] squared reach of the valid disk in x pixels (k_rotate_avg)
     DevBuf d_coef, d_k, d_reach2;
-    bool have_optics = false;
+    bool have_optics = false, optics_dirty = false;    // dirty: host tables newer than the device copies
     // angles
     int nA = 0;
     std::vector<double2> cs;
+    std::vector<float4> csf;
+    bool angles_dirty = false;
     DevBuf d_tiles[8];                          // rotate tile tables for EG = 1, 2, 4, 8 and AS = 1, 4
     DevBuf d_cs, d_csf;
     int n_tiles[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -80,9 +83,13 @@ struct cyrsoxs_ctx {
     unsigned long long null_pattern = ~0ull;
     // workspace
     DevBuf A1, A2, A3, img, twx, twy, twz, stage_out[2], red;
+    DevBuf tw2x, tw2y, tw2z;                     // per-stage twiddle tables of fft2.cuh (lengths 64 .. 2048)
     // last run
     cyrsoxs_stats stats{};
     cudaStream_t last_stream = nullptr;
+    cudaEvent_t ev_run_done = nullptr;             // end of the last run on last_stream (cross-stream reuse of the workspace)
+    bool ran = false;
+    std::vector<const void *> smem_attr_done;      // kernels whose dynamic shared-memory limit has been raised
     int last_batch_e = 0;
     std::vector<cudaEvent_t> prof_events;          // pairs (start, stop) tagged by stage
     std::vector<int> prof_stage;
@@ -117,6 +124,29 @@ cyrsoxs_status fail(cyrsoxs_ctx *c, cyrsoxs_status st, const char *fmt, ...)
                         "%s: %s", #expr, cudaGetErrorString(_e));                                 \
         }                                                                                         \
     } while (0)
+
+// Makes the context's device current for the duration of an entry point and restores the caller's.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; }
+        if (prev != dev) { switched = cudaSetDevice(dev) == cudaSuccess; if (!switched) cudaGetLastError(); }
+    }
+    ~DeviceGuard() { if (switched && prev >= 0) cudaSetDevice(prev); }
+};
+
+// Raises a kernel's dynamic shared-memory limit once per context (a context is used by one host thread).
+template <class K> cyrsoxs_status allow_smem(cyrsoxs_ctx *c, K kernel, size_t bytes)
+{
+    const void *f = reinterpret_cast<const void *>(kernel);
+    if (bytes <= 48 * 1024 || std::find(c->smem_attr_done.begin(), c->smem_attr_done.end(), f) != c->smem_attr_done.end())
+        return CYRSOXS_OK;
+    CUDA_TRY(c, cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    c->smem_attr_done.push_back(f);
+    return CYRSOXS_OK;
+}
 
 bool is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
 int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
@@ -158,6 +188,22 @@ cyrsoxs_status make_twiddles(cyrsoxs_ctx *c, DevBuf &b, int N)
     return CYRSOXS_OK;
 }
 
+// Per-stage twiddle tables of fft2.cuh for a power-of-two length 64 .. 2048 (nothing for other lengths).
+cyrsoxs_status make_twiddles2(cyrsoxs_ctx *c, DevBuf &b, int N)
+{
+    std::vector<float2> h;
+    switch (is_pow2(N) ? ilog2(N) : 0) {
+#define CASE(L) case L: h.resize(Fft2<L>::TW_TOTAL); fft2_fill_twiddles<L>(h.data()); break;
+        CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11)
+#undef CASE
+    default: return CYRSOXS_OK;
+    }
+    cyrsoxs_status st = ensure(c, b, sizeof(float2) * h.size());
+    if (st != CYRSOXS_OK) return st;
+    CUDA_TRY(c, cudaMemcpy(b.p, h.data(), sizeof(float2) * h.size(), cudaMemcpyHostToDevice));
+    return CYRSOXS_OK;
+}
+
 // Window of bins [-K, K] (symmetric) or [-K, 0] (one-sided) on an axis of length N.
 Window make_window(int N, int K, bool symmetric)
 {
@@ -179,7 +225,7 @@ template <int AS> void rot_tile_dims(int lg, int &TW, int &TH)
     TH = lg == 0 ? RotMap<1, AS>::TH : lg == 1 ? RotMap<2, AS>::TH : lg == 2 ? RotMap<4, AS>::TH : RotMap<8, AS>::TH;
 }
 
-cyrsoxs_status make_rotate_tiles(cyrsoxs_ctx *c, int lg, int as)
+cyrsoxs_status make_rotate_tiles(cyrsoxs_ctx *c, cudaStream_t stream, int lg, int as)
 {
     const int slot = lg + (as == 4 ? 4 : 0);
     if (c->n_tiles[slot]) return CYRSOXS_OK;
@@ -199,7 +245,8 @@ cyrsoxs_status make_rotate_tiles(cyrsoxs_ctx *c, int lg, int as)
     for (size_t i = 0; i < t.size(); ++i) h[i] = t[i].second;
     cyrsoxs_status st = ensure(c, c->d_tiles[slot], sizeof(uint32_t) * h.size());
     if (st != CYRSOXS_OK) return st;
-    CUDA_TRY(c, cudaMemcpy(c->d_tiles[slot].p, h.data(), sizeof(uint32_t) * h.size(), cudaMemcpyHostToDevice));
+    // pageable source: staged by the driver before the call returns, stream-ordered on the device
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_tiles[slot].p, h.data(), sizeof(uint32_t) * h.size(), cudaMemcpyHostToDevice, stream));
     c->n_tiles[slot] = (int)h.size();
     return CYRSOXS_OK;
 }
@@ -208,8 +255,6 @@ cyrsoxs_status make_rotate_tiles(cyrsoxs_ctx *c, int lg, int as)
 // whose padding (lanes of the last group without an energy) stays below a third, else 1.
 int choose_eg(int eb)
 {
-    static const int force = getenv("CYRSOXS_EG") ? atoi(getenv("CYRSOXS_EG")) : 0;      // tuning aid
-    if (force == 1 || force == 2 || force == 4 || force == 8) return force;
     for (int eg = 8; eg >= 2; eg >>= 1) {
         const int padded = (eb + eg - 1) / eg * eg;
         if (3 * (padded - eb) <= padded) return eg;
@@ -233,11 +278,7 @@ template <int LOGN> cyrsoxs_status launch_xpass_t(cyrsoxs_ctx *c, cudaStream_t s
                                                   const Window &wx, int pitch)
 {
     using Cfg = XCfg<LOGN>;
-    static bool attr_done[64] = {false};
-    if (!attr_done[c->device & 63]) {
-        CUDA_TRY(c, cudaFuncSetAttribute(k_xpass_chi<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-        attr_done[c->device & 63] = true;
-    }
+    if (cyrsoxs_status a = allow_smem(c, k_xpass_chi<LOGN>, Cfg::SMEM)) return a;
     const int rows = c->Ny * c->Nz;
     dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS, eb);
     k_xpass_chi<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(c->mp, (const float *)c->d_coef.p, e0, out, rows, wx, pitch,
@@ -259,12 +300,7 @@ cyrsoxs_status launch_xpass(cyrsoxs_ctx *c, cudaStream_t st, int e0, int eb, flo
 template <int LOGN> cyrsoxs_status launch_colpass_t(cyrsoxs_ctx *c, cudaStream_t st, ColParams p, int n_lo, int n_hi, int pitch)
 {
     using Cfg = Col2Cfg<LOGN>;
-    static bool attr_done[64] = {false};
-    if (!attr_done[c->device & 63]) {
-        if (Cfg::SMEM > 48 * 1024)
-            CUDA_TRY(c, cudaFuncSetAttribute(k_col2<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-        attr_done[c->device & 63] = true;
-    }
+    if (cyrsoxs_status a = allow_smem(c, k_col2<LOGN>, Cfg::SMEM)) return a;
     p.n_tiles = pitch / Cfg::TX;
     dim3 grid((unsigned)(p.n_tiles * n_lo), (unsigned)n_hi);
     k_col2<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
@@ -275,11 +311,7 @@ template <int LOGN> cyrsoxs_status launch_colpass_t(cyrsoxs_ctx *c, cudaStream_t
 template <int LOGN, int PW> cyrsoxs_status launch_colpass_pair_t(cyrsoxs_ctx *c, cudaStream_t st, ColParams p, int n_lo, int n_hi, int pitch)
 {
     using Cfg = Col2PCfg<LOGN, PW>;
-    static bool attr_done[64] = {false};
-    if (!attr_done[c->device & 63]) {
-        CUDA_TRY(c, cudaFuncSetAttribute(k_col2p<LOGN, PW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-        attr_done[c->device & 63] = true;
-    }
+    if (cyrsoxs_status a = allow_smem(c, k_col2p<LOGN, PW>, Cfg::SMEM)) return a;
     p.n_tiles = pitch / Cfg::TX;
     dim3 grid((unsigned)(p.n_tiles * n_lo), (unsigned)n_hi);
     k_col2p<LOGN, PW><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
@@ -292,12 +324,7 @@ cyrsoxs_status launch_colpass(cyrsoxs_ctx *c, cudaStream_t st, int N, const ColP
     if (!is_pow2(N)) {
         // a z axis of any length (DESIGN 3-A14): the pruned direct DFT
         const size_t smem = sizeof(float2) * ((size_t)N * DFT_TX + N);
-        static bool attr_done[64] = {false};
-        if (!attr_done[c->device & 63]) {
-            CUDA_TRY(c, cudaFuncSetAttribute(k_coldft, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)(sizeof(float2) * ((size_t)kMaxNzAny * DFT_TX + kMaxNzAny))));
-            attr_done[c->device & 63] = true;
-        }
+        if (cyrsoxs_status a = allow_smem(c, k_coldft, sizeof(float2) * ((size_t)kMaxNzAny * DFT_TX + kMaxNzAny))) return a;
         ColParams q = p;
         q.n_tiles = pitch / DFT_TX;
         dim3 grid((unsigned)(q.n_tiles * n_lo), (unsigned)n_hi);
@@ -307,8 +334,21 @@ cyrsoxs_status launch_colpass(cyrsoxs_ctx *c, cudaStream_t st, int N, const ColP
     }
     // lengths 128 .. 1024 take the two-columns-per-thread kernel (measured faster at every one of them:
     // cfg2 z 29 -> 25 us, cfg3 z 0.75 -> 0.65 / y 0.49 -> 0.40 ms, cfg5 z 7.4 -> 4.5 / y 4.1 -> 3.1 ms)
-    static const int pair_min = getenv("CYRSOXS_PAIR_MIN") ? atoi(getenv("CYRSOXS_PAIR_MIN")) : 7;      // tuning aid
+    constexpr int pair_min = 7;
     const int lg = ilog2(N);
+#ifdef CYRSOXS_TUNING          // sweep aid, compiled out of the shipped library
+    if (const char *e = getenv("CYRSOXS_PW")) {
+        const int pw = atoi(e);
+        if (pw == 4) switch (lg) {
+            case 9: return launch_colpass_pair_t<9, 4>(c, st, p, n_lo, n_hi, pitch);
+            case 10: return launch_colpass_pair_t<10, 4>(c, st, p, n_lo, n_hi, pitch);
+        }
+        if (pw == 2) switch (lg) {
+            case 9: return launch_colpass_pair_t<9, 2>(c, st, p, n_lo, n_hi, pitch);
+            case 10: return launch_colpass_pair_t<10, 2>(c, st, p, n_lo, n_hi, pitch);
+        }
+    }
+#endif
     // all strides are multiples of 2 elements (pitch is a multiple of 32), so 128-bit accesses are aligned
     if (lg >= pair_min) {
         switch (lg) {
@@ -366,8 +406,6 @@ template <int EG> dim3 ewald_grid(const cyrsoxs_ctx *c, int eb)
 template <int EG>
 cyrsoxs_status launch_rotate_t(cyrsoxs_ctx *c, cudaStream_t st, RotateParams p, int eb, int lg)
 {
-    static const int force_ua = getenv("CYRSOXS_ROT_UA") ? atoi(getenv("CYRSOXS_ROT_UA")) : 0;      // tuning aids
-    static const int force_as = getenv("CYRSOXS_ROT_AS") ? atoi(getenv("CYRSOXS_ROT_AS")) : 0;
     // groups per CTA: all of them (up to ROT_GMAX), so the cells of an angle are computed once per pixel
     const int ng = (eb + EG - 1) / EG;
     const int gpc = std::min(ng, ROT_GMAX);
@@ -377,8 +415,7 @@ cyrsoxs_status launch_rotate_t(cyrsoxs_ctx *c, cudaStream_t st, RotateParams p, 
     // several energy groups to walk through per angle (cfg2: 38 -> 35 us; no gain on cfg1's single energy)
     const long long px_ctas = ((long long)c->Nx * c->Ny * EG + 255) / 256 * slices_y;
     int as = (px_ctas < 4LL * c->n_sm && c->nA >= 8 && ng >= 2) ? 4 : 1;
-    if (force_as == 1 || force_as == 4) as = force_as;
-    cyrsoxs_status s = make_rotate_tiles(c, lg, as);
+    cyrsoxs_status s = make_rotate_tiles(c, st, lg, as);
     if (s != CYRSOXS_OK) return s;
     const int slot = lg + (as == 4 ? 4 : 0);
     p.tiles = (const uint32_t *)c->d_tiles[slot].p;
@@ -386,7 +423,7 @@ cyrsoxs_status launch_rotate_t(cyrsoxs_ctx *c, cudaStream_t st, RotateParams p, 
     const size_t smem = (size_t)gpc * 256 * 8;
     // angles in flight: 1 when the grid fills the machine several times over (occupancy hides the
     // load latency; measured best on cfg4), more when it does not
-    const int ua = force_ua ? force_ua : ((long long)grid.x * grid.y >= 16LL * c->n_sm ? 1 : (as == 4 ? 2 : 4));
+    const int ua = (long long)grid.x * grid.y >= 16LL * c->n_sm ? 1 : (as == 4 ? 2 : 4);
     if (as == 4) {
         if (ua == 4) k_rotate_avg<EG, 4, 2, 4><<<grid, 256, smem, st>>>(p);
         else if (ua == 2) k_rotate_avg<EG, 2, 3, 4><<<grid, 256, smem, st>>>(p);
@@ -489,12 +526,7 @@ cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int
 template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch)
 {
     using Cfg = XB2Cfg<LOGN>;
-    static bool attr_done[64] = {false};
-    if (!attr_done[c->device & 63]) {
-        if (Cfg::SMEM > 48 * 1024)
-            CUDA_TRY(c, cudaFuncSetAttribute(k_xbasis2<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-        attr_done[c->device & 63] = true;
-    }
+    if (cyrsoxs_status a = allow_smem(c, k_xbasis2<LOGN>, Cfg::SMEM)) return a;
     const int rows = c->Ny * c->Nz;
     dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS);
     k_xbasis2<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(mp, out, rows, wx, pitch, (const float2 *)c->twx.p);
@@ -502,14 +534,62 @@ template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t 
     return CYRSOXS_OK;
 }
 
+template <int LOGN> cyrsoxs_status launch_xbasis3_t(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch)
+{
+    using Cfg = XB3Cfg<LOGN>;
+    if (cyrsoxs_status a = allow_smem(c, k_xbasis3<LOGN>, Cfg::SMEM)) return a;
+    const int rows = c->Ny * c->Nz;
+    dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS);
+    size_t smem = Cfg::SMEM;
+#ifdef CYRSOXS_TUNING          // sweep aid, compiled out of the shipped library: occupancy sensitivity
+    if (const char *e = getenv("CYRSOXS_XB3_SMEM")) { smem = std::max(smem, (size_t)atoi(e)); cudaFuncSetAttribute(k_xbasis3<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); }
+#endif
+    int ahead = c->n_sm * Cfg::MINB * Cfg::ROWS;               // rows in flight on the whole GPU
+#ifdef CYRSOXS_TUNING
+    if (const char *e = getenv("CYRSOXS_XB3_AHEAD")) ahead = atoi(e);
+#endif
+    k_xbasis3<LOGN><<<grid, Cfg::THREADS, smem, st>>>(mp, out, rows, (size_t)rows * pitch, wx, pitch, (const float2 *)c->tw2x.p, ahead);
+    CUDA_TRY(c, cudaGetLastError());
+    return CYRSOXS_OK;
+}
+
 cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch)
 {
     switch (ilog2(c->Nx)) {
+#define CASE3(L) case L: return launch_xbasis3_t<L>(c, st, mp, out, wx, pitch);
+        CASE3(6) CASE3(7) CASE3(8) CASE3(9) CASE3(10) CASE3(11)
+#undef CASE3
 #define CASE(L) case L: return launch_xbasis_t<L>(c, st, mp, out, wx, pitch);
-        CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11)
+        CASE(2) CASE(3) CASE(4) CASE(5)
 #undef CASE
     }
     return fail(c, CYRSOXS_ERR_INVALID_ARG, "unsupported Nx");
+}
+
+// Device copies of the small host tables (per-energy coefficients and wavenumbers, per-angle cos/sin) are refreshed
+// at cyrsoxs_run, on the run's stream: a setter called while an earlier run is still executing cannot overwrite what
+// that run's kernels read (the copies are ordered after it on the stream).  Pageable sources are staged by the
+// driver before cudaMemcpyAsync returns, so the host vectors may change right afterwards.
+cyrsoxs_status upload_tables(cyrsoxs_ctx *c, cudaStream_t st)
+{
+    cyrsoxs_status s;
+    if (c->optics_dirty) {
+        if ((s = ensure(c, c->d_coef, sizeof(float) * c->coef.size())) != CYRSOXS_OK) return s;
+        if ((s = ensure(c, c->d_k, sizeof(double) * c->k.size())) != CYRSOXS_OK) return s;
+        if ((s = ensure(c, c->d_reach2, sizeof(float) * c->reach2.size())) != CYRSOXS_OK) return s;
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_coef.p, c->coef.data(), sizeof(float) * c->coef.size(), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_k.p, c->k.data(), sizeof(double) * c->k.size(), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_reach2.p, c->reach2.data(), sizeof(float) * c->reach2.size(), cudaMemcpyHostToDevice, st));
+        c->optics_dirty = false;
+    }
+    if (c->angles_dirty) {
+        if ((s = ensure(c, c->d_cs, sizeof(double2) * c->cs.size())) != CYRSOXS_OK) return s;
+        if ((s = ensure(c, c->d_csf, sizeof(float4) * c->csf.size())) != CYRSOXS_OK) return s;
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_cs.p, c->cs.data(), sizeof(double2) * c->cs.size(), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_csf.p, c->csf.data(), sizeof(float4) * c->csf.size(), cudaMemcpyHostToDevice, st));
+        c->angles_dirty = false;
+    }
+    return CYRSOXS_OK;
 }
 
 // Is material m aligned (has S, theta, psi)?  In streamed mode the host table decides.
@@ -518,7 +598,7 @@ bool is_aligned(const cyrsoxs_ctx *c, int m) { return (c->streamed ? c->host_mp.
 // The basis fields in material order (7 per aligned, 1 per isotropic material), two per complex
 // pack, the last pack padded; the per-field kind/material tables and the per-energy complex
 // coefficient of each field (times 1/2 for the unpacking).
-cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c)
+cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c, cudaStream_t st)
 {
     c->basis_kind.clear(); c->basis_mat.clear();
     for (int m = 0; m < c->n_mat; ++m) {
@@ -549,8 +629,9 @@ cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c)
     cyrsoxs_status s;
     if ((s = ensure(c, c->d_bcoef, sizeof(float2) * coef.size())) != CYRSOXS_OK) return s;
     if ((s = ensure(c, c->d_bkind, sizeof(int) * nb)) != CYRSOXS_OK) return s;
-    CUDA_TRY(c, cudaMemcpy(c->d_bcoef.p, coef.data(), sizeof(float2) * coef.size(), cudaMemcpyHostToDevice));
-    CUDA_TRY(c, cudaMemcpy(c->d_bkind.p, c->basis_kind.data(), sizeof(int) * nb, cudaMemcpyHostToDevice));
+    // pageable sources: staged by the driver before these calls return; ordered after the stream's earlier work
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_bcoef.p, coef.data(), sizeof(float2) * coef.size(), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_bkind.p, c->basis_kind.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
     c->plan_dirty = false;
     return CYRSOXS_OK;
 }
@@ -654,9 +735,8 @@ cyrsoxs_status run_batch_spectral(cyrsoxs_ctx *c, cudaStream_t st, int e0, int e
         p.wx = wx; p.wy = wy; p.wz = wz; p.pitch = pitch;
         p.spec = (const float2 *)c->A3.p; p.img = (float4 *)c->img.p;
         q.n_pack = c->n_pack; q.coef = (const float2 *)c->d_bcoef.p; q.kind = (const int *)c->d_bkind.p;
-        static const int no_2d = getenv("CYRSOXS_NO_EW2D") ? atoi(getenv("CYRSOXS_NO_EW2D")) : 0;      // tuning aid
         const size_t smem2d = (size_t)eb * (2 * sizeof(double) + sizeof(float) + 2 * c->n_pack * sizeof(float2)) + 2 * c->n_pack * sizeof(int);
-        if (c->Nz == 1 && eb >= 4 && c->n_pack <= EW2D_MAXP && smem2d <= 48 * 1024 && !no_2d) {
+        if (c->Nz == 1 && eb >= 4 && c->n_pack <= EW2D_MAXP && smem2d <= 48 * 1024) {
             // 2-D model, several energies: one thread per pixel, the batch's energies in an inner loop (see
             // k_ewald_basis_2d; cfg4 15.8 -> 6.6 ms; a single energy is better off with a thread per energy)
             const dim3 g2d((c->Nx + 31) / 32, (c->Ny + 7) / 8);
@@ -710,7 +790,8 @@ cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm,
     if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); c->n_sm = 148; }
     cyrsoxs_status st;
     if ((st = make_twiddles(c, c->twx, Nx)) != CYRSOXS_OK || (st = make_twiddles(c, c->twy, Ny)) != CYRSOXS_OK
-        || (st = make_twiddles(c, c->twz, Nz)) != CYRSOXS_OK) {
+        || (st = make_twiddles(c, c->twz, Nz)) != CYRSOXS_OK || (st = make_twiddles2(c, c->tw2x, Nx)) != CYRSOXS_OK
+        || (st = make_twiddles2(c, c->tw2y, Ny)) != CYRSOXS_OK || (st = make_twiddles2(c, c->tw2z, Nz)) != CYRSOXS_OK) {
         cyrsoxs_destroy(c);
         return st;
     }
@@ -721,9 +802,11 @@ cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm,
 void cyrsoxs_destroy(cyrsoxs_ctx *c)
 {
     if (!c) return;
+    DeviceGuard guard(c->device);
+    cudaDeviceSynchronize();                 // nothing of this context may still be running when its buffers go
     clear_prof(c);
     for (void *p : c->owned_morph) cudaFree(p);
-    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->d_tiles[4], &c->d_tiles[5], &c->d_tiles[6], &c->d_tiles[7], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz,
+    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->d_tiles[4], &c->d_tiles[5], &c->d_tiles[6], &c->d_tiles[7], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz, &c->tw2x, &c->tw2y, &c->tw2z,
                       &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind, &c->red})
         release(*b);
     release(c->stage_morph[0]); release(c->stage_morph[1]);
@@ -732,6 +815,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
         if (c->ev_stage_free[i]) cudaEventDestroy(c->ev_stage_free[i]);
     }
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->ev_run_done) cudaEventDestroy(c->ev_run_done);
     for (int i = 0; i < 2; ++i) {
         if (c->ev_batch[i]) cudaEventDestroy(c->ev_batch[i]);
         if (c->ev_copy[i]) cudaEventDestroy(c->ev_copy[i]);
@@ -778,6 +862,13 @@ cyrsoxs_status cyrsoxs_set_morphology(cyrsoxs_ctx *c, const float *const *d_phi,
         c->mp.psi[m] = d_psi ? d_psi[m] : nullptr;
     }
     c->streamed = false;
+    if (!c->owned_morph.empty()) {
+        // device copies left by an earlier cyrsoxs_set_morphology_host / _aos (cudaFree waits for the work that reads them)
+        DeviceGuard guard(c->device);
+        for (void *p : c->owned_morph) cudaFree(p);
+        c->owned_morph.clear();
+        c->plan_eb = 0;                      // the energy batch was planned with less free memory
+    }
     note_null_pattern(c);
     c->have_morph = true;
     return CYRSOXS_OK;
@@ -790,6 +881,9 @@ cyrsoxs_status cyrsoxs_set_morphology_host(cyrsoxs_ctx *c, const float *const *h
     cyrsoxs_status st = check_morph_tables(c, h_phi, h_S, h_theta, h_psi);
     if (st != CYRSOXS_OK) return st;
     cudaStream_t s = (cudaStream_t)cuda_stream;
+    DeviceGuard guard(c->device);
+    // an earlier run on another stream may still be reading the buffers this call overwrites
+    if (c->ran && s != c->last_stream) CUDA_TRY(c, cudaStreamWaitEvent(s, c->ev_run_done, 0));
     const size_t bytes = sizeof(float) * (size_t)c->Nx * c->Ny * c->Nz;
     // count arrays, (re)allocate owned buffers
     std::vector<const float *> src;
@@ -853,8 +947,11 @@ cyrsoxs_status cyrsoxs_set_morphology_streamed(cyrsoxs_ctx *c, const float *cons
     c->host_mp.n_mat = c->n_mat;
     c->streamed = true;
     c->stream_group = std::min(materials_per_group, c->n_mat);
-    for (void *p : c->owned_morph) cudaFree(p);
-    c->owned_morph.clear();
+    {
+        DeviceGuard guard(c->device);
+        for (void *p : c->owned_morph) cudaFree(p);
+        c->owned_morph.clear();
+    }
     c->plan_dirty = true;
     note_null_pattern(c);
     c->have_morph = true;
@@ -867,7 +964,8 @@ cyrsoxs_status cyrsoxs_set_morphology_aos(cyrsoxs_ctx *c, const float *d_real4, 
     if (!d_real4) return fail(c, CYRSOXS_ERR_INVALID_ARG, "morphology array is NULL");
     if ((uintptr_t)d_real4 & 15) return fail(c, CYRSOXS_ERR_INVALID_ARG, "morphology array not 16-byte aligned");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    CUDA_TRY(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    if (c->ran && st != c->last_stream) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_run_done, 0));
     const size_t n = (size_t)c->Nx * c->Ny * c->Nz, bytes = sizeof(float) * n;
     const size_t need = 4 * (size_t)c->n_mat;
     if (c->owned_morph.size() != need) {
@@ -949,23 +1047,18 @@ cyrsoxs_status cyrsoxs_set_optical_constants(cyrsoxs_ctx *c, int n_energy, const
             o[4] = (float)Cb.real(); o[5] = (float)Cb.imag();
         }
     }
-    cyrsoxs_status st;
-    if ((st = ensure(c, c->d_coef, sizeof(float) * c->coef.size())) != CYRSOXS_OK) return st;
-    if ((st = ensure(c, c->d_k, sizeof(double) * n_energy)) != CYRSOXS_OK) return st;
-    CUDA_TRY(c, cudaMemcpy(c->d_coef.p, c->coef.data(), sizeof(float) * c->coef.size(), cudaMemcpyHostToDevice));
-    CUDA_TRY(c, cudaMemcpy(c->d_k.p, c->k.data(), sizeof(double) * n_energy, cudaMemcpyHostToDevice));
     {
         // reach of the valid disk in x pixels, see k_rotate_avg
-        std::vector<float> reach2(n_energy);
+        c->reach2.resize(n_energy);
         const double rho = (double)c->Nx / (double)c->Ny;
         for (int e = 0; e < n_energy; ++e) {
             const double r = c->k[e] / c->dqx + sqrt(1.0 + rho * rho) + 1.0;
-            reach2[e] = (float)(r * r * 1.0001);
+            c->reach2[e] = (float)(r * r * 1.0001);
         }
-        if ((st = ensure(c, c->d_reach2, sizeof(float) * n_energy)) != CYRSOXS_OK) return st;
-        CUDA_TRY(c, cudaMemcpy(c->d_reach2.p, reach2.data(), sizeof(float) * n_energy, cudaMemcpyHostToDevice));
     }
+    // the device copies are refreshed by the next cyrsoxs_run, on its stream (a run still executing keeps its tables)
     c->have_optics = true;
+    c->optics_dirty = true;
     c->plan_dirty = true;
     return CYRSOXS_OK;
 }
@@ -986,7 +1079,8 @@ cyrsoxs_status cyrsoxs_set_angles(cyrsoxs_ctx *c, double start_deg, double step_
     }
     c->nA = n;
     c->cs.resize(n);
-    std::vector<float4> csf(n);
+    std::vector<float4> &csf = c->csf;
+    csf.resize(n);
     for (int i = 0; i < n; ++i) {
         const double zeta = start_deg + (double)i * step_deg;
         const double zr = zeta * (kPi / 180.0);
@@ -996,12 +1090,8 @@ cyrsoxs_status cyrsoxs_set_angles(cyrsoxs_ctx *c, double start_deg, double step_
         c->cs[i] = make_double2(C, S);
         csf[i] = make_float4((float)(C * C), (float)(S * S), (float)(2.0 * C * S), 0.f);
     }
-    cyrsoxs_status st;
-    if ((st = ensure(c, c->d_cs, sizeof(double2) * n)) != CYRSOXS_OK) return st;
-    if ((st = ensure(c, c->d_csf, sizeof(float4) * n)) != CYRSOXS_OK) return st;
-    CUDA_TRY(c, cudaMemcpy(c->d_cs.p, c->cs.data(), sizeof(double2) * n, cudaMemcpyHostToDevice));
-    CUDA_TRY(c, cudaMemcpy(c->d_csf.p, csf.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
     c->have_angles = true;
+    c->angles_dirty = true;
     return CYRSOXS_OK;
 }
 
@@ -1046,7 +1136,10 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
         return fail(c, CYRSOXS_ERR_NOT_READY, "run needs morphology, optical constants and angles (missing:%s%s%s)",
                     c->have_morph ? "" : " morphology", c->have_optics ? "" : " optical-constants", c->have_angles ? "" : " angles");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    CUDA_TRY(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    if (!c->ev_run_done) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_run_done, cudaEventDisableTiming));
+    // the workspace and the device tables are shared by consecutive runs: a run on another stream waits for the last one
+    if (c->ran && st != c->last_stream) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_run_done, 0));
 
     // where does `out` live?
     cudaPointerAttributes pa{};
@@ -1057,7 +1150,8 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
         return fail(c, CYRSOXS_ERR_INVALID_ARG, "out must be device memory or pinned host memory");
 
     cyrsoxs_status s;
-    if (c->plan_dirty && (s = build_basis_plan(c)) != CYRSOXS_OK) return s;
+    if ((s = upload_tables(c, st)) != CYRSOXS_OK) return s;
+    if (c->plan_dirty && (s = build_basis_plan(c, st)) != CYRSOXS_OK) return s;
     // AUTO: the basis needs n_pack complex transforms per run, PER_ENERGY 5 per energy; a basis transform
     // (register-first x pass, real fields) costs about half of a PER_ENERGY one (measured on cfg3: 0.31 ms
     // per pack against 0.6 ms per field), hence the factor 2
@@ -1077,7 +1171,8 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     const size_t a1 = F1 * c->Nz * c->Ny * pitch, a2 = c->Nz > 1 ? F1 * wz.W * c->Ny * pitch : 0, a3 = F1 * wz.W * wy.W * pitch;
     const size_t per_img = sizeof(float4) * npix + (out_on_host ? 2 * sizeof(float) * npix : 0);
     const size_t per_e = spectral ? per_img : sizeof(float2) * (a1 + a2 + a3) + per_img;
-    const size_t fixed = spectral ? sizeof(float2) * (a1 + a2 + a3) : 0;
+    const size_t stage_bytes = c->streamed ? 2 * (size_t)c->stream_group * 4 * sizeof(float) * (size_t)c->Nx * c->Ny * c->Nz : 0;
+    const size_t fixed = (spectral ? sizeof(float2) * (a1 + a2 + a3) : 0) + stage_bytes;
     // The energy batch depends on the free device memory; cudaMemGetInfo is slow, so the batch is
     // re-planned only when what it depends on has changed since the last run.
     const unsigned long long plan_key = (unsigned long long)c->nE * 8 + (spectral ? 4 : 0) + (out_on_host ? 2 : 0) + 1;
@@ -1085,7 +1180,8 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     if (plan_key != c->plan_key || fixed != c->plan_fixed || per_e != c->plan_per_e || eb < 1) {
         size_t free_b = 0, total_b = 0;
         CUDA_TRY(c, cudaMemGetInfo(&free_b, &total_b));
-        const size_t have = c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap;
+        const size_t have = c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap
+                            + c->stage_morph[0].cap + c->stage_morph[1].cap;
         const size_t budget = (size_t)((double)(free_b + have) * 0.85);
         if (fixed + per_e > budget)
             return fail(c, CYRSOXS_ERR_OOM, "workspace of %.1f GB does not fit in %.1f GB of free device memory",
@@ -1154,6 +1250,8 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
         // `out` is complete when `st` reaches this point
         for (int i = 0; i < std::min(nb, 2); ++i) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_copy[i], 0));
     }
+    CUDA_TRY(c, cudaEventRecord(c->ev_run_done, st));
+    c->ran = true;
     return CYRSOXS_OK;
 }
 
@@ -1161,6 +1259,7 @@ cyrsoxs_status cyrsoxs_get_stats(cyrsoxs_ctx *c, cyrsoxs_stats *stats)
 {
     if (!c || !stats) return CYRSOXS_ERR_INVALID_ARG;
     if (c->profiling && !c->prof_events.empty()) {
+        DeviceGuard guard(c->device);
         CUDA_TRY(c, cudaStreamSynchronize(c->last_stream));
         for (int i = 0; i < CYRSOXS_N_STAGES; ++i) c->stats.stage_ms[i] = 0.f;
         for (size_t i = 0; i < c->prof_stage.size(); ++i) {
@@ -1182,7 +1281,7 @@ cyrsoxs_status cyrsoxs_reduce(cyrsoxs_ctx *c, void *cuda_stream, const float *d_
     if (!(sector_half_width_deg > 0.0) || !(sector_half_width_deg <= 45.0))
         return fail(c, CYRSOXS_ERR_INVALID_ARG, "reduce: sector half width must be in (0, 45] degrees");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    CUDA_TRY(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
     const size_t nb = (size_t)n_energy * 3 * n_bins;
     const size_t bytes = sizeof(double) * nb + sizeof(double) * n_energy + sizeof(unsigned int) * nb;
     cyrsoxs_status s = ensure(c, c->red, bytes);
@@ -1199,11 +1298,8 @@ cyrsoxs_status cyrsoxs_reduce(cyrsoxs_ctx *c, void *cuda_stream, const float *d_
     p.rows_per_cta = std::max(4, (c->Ny + want - 1) / want);
     const dim3 grid((c->Ny + p.rows_per_cta - 1) / p.rows_per_cta, n_energy);
     const size_t smem = (size_t)3 * n_bins * (sizeof(double) + sizeof(unsigned int));
-    static bool attr_done[64] = {false};
-    if (smem > 48 * 1024 && !attr_done[c->device & 63]) {
-        CUDA_TRY(c, cudaFuncSetAttribute(k_reduce_accumulate, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 4096 * 12));
-        attr_done[c->device & 63] = true;
-    }
+    if (smem > 48 * 1024)
+        if (cyrsoxs_status a = allow_smem(c, k_reduce_accumulate, (size_t)3 * 4096 * 12)) return a;
     k_reduce_accumulate<<<grid, 256, smem, st>>>(p);
     CUDA_TRY(c, cudaGetLastError());
     const int tot = n_energy * n_bins;
@@ -1216,6 +1312,7 @@ cyrsoxs_status cyrsoxs_debug_fetch_images(cyrsoxs_ctx *c, int e_in_batch, float 
 {
     if (!c || !d_dst) return CYRSOXS_ERR_INVALID_ARG;
     if (!c->img.p || e_in_batch < 0 || e_in_batch >= c->last_batch_e) return fail(c, CYRSOXS_ERR_INVALID_ARG, "no such image");
+    DeviceGuard guard(c->device);
     const size_t npix = (size_t)c->Nx * c->Ny;
     const int eg = c->eg;
     const float4 *src = (const float4 *)c->img.p + (size_t)(e_in_batch / eg) * npix * eg + e_in_batch % eg;

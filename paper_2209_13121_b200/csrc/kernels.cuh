@@ -519,10 +519,10 @@ template <int EG, int AS> struct RotMap {
     static constexpr int TW = WSX * WPW, TH = WSY * WPH;                      // CTA tile
 };
 
-// reach2[e] = (k_e/dq_x + 3)^2: an output pixel whose distance from q = 0 (measured in x
+// reach2[e] = (k_e/dq_x + sqrt(1 + rho^2) + 1)^2 (+ 0.01 %): an output pixel whose distance from q = 0 (measured in x
 // pixels, y pixels scaled by rho) exceeds the reach has every bilinear neighbour outside the
 // Ewald disk s^2 >= 0 at every angle (rotation keeps the distance, a cell adds < 2 pixels), so
-// its count is 0 and nothing needs to be read.  The margin of 3 keeps the decision away from
+// its count is 0 and nothing needs to be read.  The margin (cell diagonal + 1) keeps the decision away from
 // rounding: only pixels that are invalid with certainty are skipped.
 //
 // Loop order: angles in chunks of UA; the chunk's cells are computed once (registers) and

@@ -2,6 +2,7 @@
 // register-last): the strided z / y pass (k_col2) and the SPECTRAL_BASIS x pass (k_xbasis2).
 #pragma once
 #include "fft_reg.cuh"
+#include "fft2.cuh"
 #include "kernels.cuh"
 
 namespace cyr {
@@ -184,6 +185,22 @@ k_coldft(const ColParams p, int N)
 // owns the voxels x = li + s T (s < R0), generates their fields in registers, runs the stage-0
 // butterfly there, and the remaining stages through a 4-pack shared-memory buffer per row; the
 // last stage stores the window [lo, lo + W) of bins straight to out[pack][row][slot].
+// sin and cos of a director angle.  CYRSOXS_TRIG = 0: libdevice sincosf (1 ulp; ~50 instructions per call with a
+// slow path for large arguments); 1: the special-function unit (MUFU.SIN / MUFU.COS after one multiplication by
+// 1/2pi: absolute error ~5e-7 for |x| up to a few pi, 4 instructions).  DESIGN.md 8 derives why 5e-7 on the director
+// is far inside the image gates; the parity tests run with whatever is compiled in.
+#ifndef CYRSOXS_TRIG
+#define CYRSOXS_TRIG 1
+#endif
+__device__ __forceinline__ void dir_sincos(float x, float *s, float *c)
+{
+#if CYRSOXS_TRIG == 0
+    sincosf(x, s, c);
+#else
+    *s = __sinf(x); *c = __cosf(x);
+#endif
+}
+
 constexpr int XB2_PB = 4;       // packs buffered per row between flushes
 static_assert(XB2_PB >= 4, "an aligned material emits up to 4 packs between flush checks");
 // CTAs per SM the register allocation aims at: 3 (80 registers, a few spilled values) measured 9-12 % faster
@@ -222,14 +239,22 @@ k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
     bool has_carry = false;
     int nbuf = 0, pack_out = 0;
 
+    // The thread's outputs are the bins k = li + T m; bin k goes to slot (k - lo) mod N when that is inside the row
+    // (slots [W, pitch) are the row's zero padding).  Slot offsets, a store mask and a zero mask are worked out once.
+    int soff[R0];
+    unsigned int st_mask = 0, zero_mask = 0;
+#pragma unroll
+    for (int m = 0; m < R0; ++m) {
+        const int sl = (li + T * m - wx.lo) & (N - 1);
+        soff[m] = sl;
+        if (sl < pitch && row_ok) st_mask |= 1u << m;
+        if (sl >= wx.W) zero_mask |= 1u << m;
+    }
     auto store_global = [&](int pack, const float2 (&v)[R0]) {
         float2 *o = orow + (size_t)pack * fstride;
 #pragma unroll
-        for (int m = 0; m < R0; ++m) {
-            const int k = li + T * m;
-            const int sl = (k - wx.lo) & (N - 1);
-            if (sl < pitch && row_ok) o[sl] = sl < wx.W ? v[F::out_reg(m)] : make_float2(0.f, 0.f);
-        }
+        for (int m = 0; m < R0; ++m)
+            if (st_mask >> m & 1u) o[soff[m]] = (zero_mask >> m & 1u) ? make_float2(0.f, 0.f) : v[F::out_reg(m)];
         if (N < 32) {
             for (int sl = N + li; sl < pitch; sl += T)
                 if (row_ok) o[sl] = make_float2(0.f, 0.f);
@@ -297,8 +322,8 @@ k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
             for (int s = 0; s < R0; ++s) {
                 w[s] = ph[s] * S_[s];
                 float st, ct, sp, cp;
-                sincosf(th[s], &st, &ct);
-                sincosf(ps[s], &sp, &cp);
+                dir_sincos(th[s], &st, &ct);
+                dir_sincos(ps[s], &sp, &cp);
                 dx[s] = cp * st; dy[s] = sp * st; dz[s] = ct;
             }
             auto f_ph = [&](int s) { return ph[s]; };
@@ -328,6 +353,175 @@ k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
     }
     if (has_carry) {
         if (nbuf + 1 > XB2_PB) flush();
+        emit([&](int s) { return carry[s]; }, [](int) { return 0.f; });
+    }
+    flush();
+}
+
+// ------------------------------------------------------------------------------------------
+// x pass of SPECTRAL_BASIS, second generation (N = 64 .. 2048; shorter rows keep k_xbasis2).  Same fields, same
+// pack order and same output layout as k_xbasis2; what differs is how a row is transformed (fft2.cuh):
+//   * the packs buffered in shared memory go through the later stages two at a time: 16 values per thread, one
+//     barrier per pair and stage, radix 16 in the middle of 1024- and 2048-point rows (2 trips through shared
+//     memory instead of 3; 128 points: 1 instead of 2);
+//   * per-stage twiddle tables read with unit stride;
+//   * the window store works from one precomputed slot per thread (k0) and compile-time offsets;
+//   * sin / cos of the director angles on the special-function unit (dir_sincos);
+//   * the next material's rows are prefetched into L2 while the current one is transformed.
+constexpr int XB3_PB = 4;
+// CTA shape (measured on B200, CFG3 / CFG5 x pass in ms): 256 threads at 128 registers (2 CTAs/SM) 1.24 / 8.8; 128
+// threads at 128 registers (4 CTAs/SM) 1.13 / 8.0; 128 threads at 96 registers (5 CTAs/SM, a few spills) 1.21 / 7.7;
+// 80 registers (heavy spills) 1.5 / 9.3-11.  The kernel is latency bound (ncu: issue slots 52 % busy at 16 warps per
+// SM), so small CTAs -- finer-grained refill of the SM -- and the fifth CTA pay at 1024 points.
+#ifndef CYRSOXS_XB3_CTA
+#define CYRSOXS_XB3_CTA 128
+#endif
+
+template <int LOGN> struct XB3Cfg {
+    static constexpr int N = 1 << LOGN;
+    using F = Fft2<LOGN>;
+    static constexpr int T = F::T;
+    static constexpr int ROWS = T >= CYRSOXS_XB3_CTA ? 1 : CYRSOXS_XB3_CTA / T;
+    static constexpr int THREADS = ROWS * T;
+#ifdef CYRSOXS_XB3_MINB
+    static constexpr int MINB = CYRSOXS_XB3_MINB;
+#else
+    static constexpr int MINB = THREADS > 128 ? 2 : (LOGN == 10 ? 5 : 4);
+#endif
+    static constexpr int LSTRIDE = PadMap::line(N) + (N <= 128 ? 8 : 0);   // line stride: keeps the two lines of a split
+    static constexpr int RSTRIDE = XB3_PB * LSTRIDE + (N == 64 ? 8 : 0);    // stage / two rows of a half-warp on distinct banks
+    static constexpr size_t SMEM = sizeof(float2) * (size_t)ROWS * RSTRIDE;
+};
+
+template <int LOGN>
+__global__ void __launch_bounds__(XB3Cfg<LOGN>::THREADS, XB3Cfg<LOGN>::MINB)
+k_xbasis3(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, size_t fstride, Window wx, int pitch,
+          const float2 *__restrict__ tws, int rows_ahead)
+{
+    using Cfg = XB3Cfg<LOGN>;
+    using F = typename Cfg::F;
+    using Map = PadMap;
+    constexpr int N = Cfg::N, T = Cfg::T, NST = F::NST, THREADS = Cfg::THREADS, LS = Cfg::LSTRIDE;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x;
+    const int g = tid / T, li = tid % T;
+    const int row = blockIdx.x * Cfg::ROWS + g;
+    const bool row_ok = row < rows_total;
+    const int rowc = row_ok ? row : rows_total - 1;
+    float2 *Lrow = reinterpret_cast<float2 *>(smem_raw) + (size_t)g * Cfg::RSTRIDE;
+    const size_t vox0 = (size_t)rowc * N + li;
+    float2 *orow = out + (size_t)rowc * pitch;
+
+    float carry[8];
+    bool has_carry = false;
+    int nbuf = 0, pack_out = 0;
+    const int lo = wx.lo, W = wx.W;
+
+    // bin k of pack `pack` goes to slot (k - lo) mod N if that is inside the row; slots [W, pitch) are zero padding
+    auto store_bin = [&](int pack, int k, float2 val) {
+        const int sl = (k - lo) & (N - 1);
+        if (sl < pitch && row_ok) orow[(size_t)pack * fstride + sl] = sl < W ? val : make_float2(0.f, 0.f);
+    };
+    auto emit = [&](auto fa, auto fb) {
+        float2 v[8];
+#pragma unroll
+        for (int s = 0; s < 8; ++s) v[s] = make_float2(fa(s), fb(s));
+        F::stage0(v);
+        F::template stage0_store<Map>(Lrow + nbuf * LS, li, v);
+        ++nbuf;
+    };
+    auto flush = [&]() {
+        float2 w[8], v[16];
+        if constexpr (NST > 2) {
+            group_sync<T, THREADS>(g);
+            F::template load_tw<1>(tws, li, w);
+            for (int pk = 0; pk < nbuf; pk += 2) {
+                float2 *LA = Lrow + pk * LS, *LB = LA + LS;
+                const bool hasB = pk + 1 < nbuf;
+                F::template stage_load<1, Map>(LA, LB, hasB, li, w, v);
+                group_sync<T, THREADS>(g);
+                F::template stage_store<1, Map>(LA, LB, hasB, li, v);
+            }
+        }
+        group_sync<T, THREADS>(g);
+        F::template load_tw<NST - 1>(tws, li, w);
+        for (int pk = 0; pk < nbuf; pk += 2) {
+            float2 *LA = Lrow + pk * LS, *LB = LA + LS;
+            const bool hasB = pk + 1 < nbuf;
+            F::template stage_load<NST - 1, Map>(LA, LB, hasB, li, w, v);
+            const int p0 = pack_out + pk;
+            F::for_each_output(hasB, li, v, [&](int line, int k, float2 val) { store_bin(p0 + line, k, val); });
+        }
+        group_sync<T, THREADS>(g);          // the buffer is reused by the next stage-0 stores
+        pack_out += nbuf;
+        nbuf = 0;
+    };
+    // one 128-byte line per lane: the T threads of a row cover its N floats with N / 32 prefetches per array
+    auto prefetch_row_of = [&](const float *a, int r) {
+        if (li < N / 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(a + (size_t)r * N + li * 32));
+    };
+    auto prefetch_row = [&](const float *a) { prefetch_row_of(a, rowc); };
+    // the first material of the rows a later CTA will start with (rows_ahead ~ the rows in flight on the whole GPU):
+    // that CTA's first loads then hit L2 instead of exposing the DRAM latency at the start of its short life
+    if (row + rows_ahead < rows_total) {
+        prefetch_row_of(mp.phi[0], row + rows_ahead);
+        if (mp.S[0]) { prefetch_row_of(mp.S[0], row + rows_ahead); prefetch_row_of(mp.theta[0], row + rows_ahead); prefetch_row_of(mp.psi[0], row + rows_ahead); }
+    }
+
+    for (int m = 0; m < mp.n_mat; ++m) {
+        const bool aligned = mp.S[m] != nullptr;
+        if (nbuf + (aligned ? 4 : 1) > XB3_PB) flush();
+        float ph[8];
+#pragma unroll
+        for (int s = 0; s < 8; ++s) ph[s] = __ldcs(mp.phi[m] + vox0 + (size_t)s * T);
+        if (m + 1 < mp.n_mat) {
+            prefetch_row(mp.phi[m + 1]);
+            if (mp.S[m + 1]) { prefetch_row(mp.S[m + 1]); prefetch_row(mp.theta[m + 1]); prefetch_row(mp.psi[m + 1]); }
+        }
+        if (aligned) {
+            float S_[8], th[8], ps[8];
+#pragma unroll
+            for (int s = 0; s < 8; ++s) {
+                S_[s] = __ldcs(mp.S[m] + vox0 + (size_t)s * T);
+                th[s] = __ldcs(mp.theta[m] + vox0 + (size_t)s * T);
+                ps[s] = __ldcs(mp.psi[m] + vox0 + (size_t)s * T);
+            }
+            float w[8], dx[8], dy[8], dz[8];
+#pragma unroll
+            for (int s = 0; s < 8; ++s) {
+                w[s] = ph[s] * S_[s];
+                float st, ct, sp, cp;
+                dir_sincos(th[s], &st, &ct);
+                dir_sincos(ps[s], &sp, &cp);
+                dx[s] = cp * st; dy[s] = sp * st; dz[s] = ct;
+            }
+            auto f_ph = [&](int s) { return ph[s]; };
+            auto f_w = [&](int s) { return w[s]; };
+            auto f_xx = [&](int s) { return (w[s] * dx[s]) * dx[s]; };
+            auto f_yy = [&](int s) { return (w[s] * dy[s]) * dy[s]; };
+            auto f_xy = [&](int s) { return (w[s] * dx[s]) * dy[s]; };
+            auto f_xz = [&](int s) { return (w[s] * dx[s]) * dz[s]; };
+            auto f_yz = [&](int s) { return (w[s] * dy[s]) * dz[s]; };
+            if (has_carry) {
+                emit([&](int s) { return carry[s]; }, f_ph); emit(f_w, f_xx); emit(f_yy, f_xy); emit(f_xz, f_yz);
+                has_carry = false;
+            } else {
+                emit(f_ph, f_w); emit(f_xx, f_yy); emit(f_xy, f_xz);
+#pragma unroll
+                for (int s = 0; s < 8; ++s) carry[s] = f_yz(s);
+                has_carry = true;
+            }
+        } else {
+            if (has_carry) { emit([&](int s) { return carry[s]; }, [&](int s) { return ph[s]; }); has_carry = false; }
+            else {
+#pragma unroll
+                for (int s = 0; s < 8; ++s) carry[s] = ph[s];
+                has_carry = true;
+            }
+        }
+    }
+    if (has_carry) {
+        if (nbuf + 1 > XB3_PB) flush();
         emit([&](int s) { return carry[s]; }, [](int) { return 0.f; });
     }
     flush();
