@@ -174,45 +174,67 @@ static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
 
 /* Eq. 6 along one axis written out as the definition, O(n^2), for a length that is not a
  * power of two (the paper uses Nz = 63; DESIGN.md 3-A14): X[k] = sum_j x[j] exp(-2 pi i
- * j k / n).  The phase index j k mod n is exact integer arithmetic. */
-static void dft1d_definition(cplx *x, int n, cplx *scratch)
+ * j k / n).  The phase index j k mod n is exact integer arithmetic; ph[t] = exp(-2 pi i t / n),
+ * t < n, is the table of the n distinct phases (make_phases). */
+static void dft1d_definition(cplx *x, int n, cplx *scratch, const cplx *ph)
 {
     for (int k = 0; k < n; ++k) {
         cplx acc = 0.0;
-        for (int j = 0; j < n; ++j) {
-            double ang = -2.0 * ORC_PI * (double)(((int64_t)j * k) % n) / (double)n;
-            acc += x[j] * (cos(ang) + I * sin(ang));
-        }
+        for (int j = 0; j < n; ++j) acc += x[j] * ph[((int64_t)j * k) % n];
         scratch[k] = acc;
     }
     memcpy(x, scratch, sizeof(cplx) * (size_t)n);
 }
 
-/* 3-D FFT of f[z][y][x] (x fastest), in place: Eq. 6, forward,
- * unnormalised, origin at voxel 0.  Nx and Ny must be powers of two (returns -1 otherwise);
- * Nz may be any length: a power of two takes the radix-2 FFT, anything else the definition. */
+static cplx *make_phases(int n)
+{
+    cplx *ph = (cplx *)malloc(sizeof(cplx) * (size_t)(n > 0 ? n : 1));
+    for (int t = 0; t < n; ++t) {
+        double ang = -2.0 * ORC_PI * (double)t / (double)n;
+        ph[t] = cos(ang) + I * sin(ang);
+    }
+    return ph;
+}
+
+/* one line of length n, in place: radix-2 FFT for a power of two, the definition otherwise */
+static void line_transform(cplx *x, int n, const cplx *tw, const cplx *ph, cplx *scratch)
+{
+    if (is_pow2(n)) fft1d_radix2(x, n, tw);
+    else dft1d_definition(x, n, scratch, ph);
+}
+
+/* 3-D FFT of f[z][y][x] (x fastest), in place: Eq. 6, forward, unnormalised, origin at
+ * voxel 0.  Any lengths (DESIGN.md 3-A14): an axis whose length is a power of two takes the
+ * radix-2 FFT, any other axis the definition of Eq. 6. */
 int orc_fft3(int Nx, int Ny, int Nz, cplx *f)
 {
-    if (!is_pow2(Nx) || !is_pow2(Ny) || Nz < 1) return -1;
+    if (Nx < 1 || Ny < 1 || Nz < 1) return -1;
     const int64_t sxy = (int64_t)Nx * Ny;
     cplx *twx = make_twiddles(Nx), *twy = make_twiddles(Ny), *twz = make_twiddles(Nz);
+    cplx *phx = is_pow2(Nx) ? NULL : make_phases(Nx), *phy = is_pow2(Ny) ? NULL : make_phases(Ny),
+         *phz = is_pow2(Nz) ? NULL : make_phases(Nz);
     /* along x: contiguous rows */
     if (Nx > 1) {
-#pragma omp parallel for schedule(static)
-        for (int64_t r = 0; r < (int64_t)Ny * Nz; ++r)
-            fft1d_radix2(f + r * Nx, Nx, twx);
+#pragma omp parallel
+        {
+            cplx *scr = (cplx *)malloc(sizeof(cplx) * (size_t)Nx);
+#pragma omp for schedule(static)
+            for (int64_t r = 0; r < (int64_t)Ny * Nz; ++r)
+                line_transform(f + r * Nx, Nx, twx, phx, scr);
+            free(scr);
+        }
     }
     /* along y */
     if (Ny > 1) {
 #pragma omp parallel
         {
-            cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)Ny);
+            cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)Ny * 2);
 #pragma omp for schedule(static)
             for (int64_t r = 0; r < (int64_t)Nx * Nz; ++r) {
                 int64_t z = r / Nx, x = r % Nx;
                 cplx *base = f + z * sxy + x;
                 for (int y = 0; y < Ny; ++y) buf[y] = base[(int64_t)y * Nx];
-                fft1d_radix2(buf, Ny, twy);
+                line_transform(buf, Ny, twy, phy, buf + Ny);
                 for (int y = 0; y < Ny; ++y) base[(int64_t)y * Nx] = buf[y];
             }
             free(buf);
@@ -227,14 +249,13 @@ int orc_fft3(int Nx, int Ny, int Nz, cplx *f)
             for (int64_t r = 0; r < sxy; ++r) {
                 cplx *base = f + r;
                 for (int z = 0; z < Nz; ++z) buf[z] = base[(int64_t)z * sxy];
-                if (is_pow2(Nz)) fft1d_radix2(buf, Nz, twz);
-                else dft1d_definition(buf, Nz, buf + Nz);
+                line_transform(buf, Nz, twz, phz, buf + Nz);
                 for (int z = 0; z < Nz; ++z) base[(int64_t)z * sxy] = buf[z];
             }
             free(buf);
         }
     }
-    free(twx); free(twy); free(twz);
+    free(twx); free(twy); free(twz); free(phx); free(phy); free(phz);
     return 0;
 }
 
@@ -530,7 +551,7 @@ int orc_run_energy(int Nx, int Ny, int Nz, int n_mat, double voxel,
 {
     const int64_t n_vox = (int64_t)Nx * Ny * Nz, n_pix = (int64_t)Nx * Ny;
     int n_ang = orc_num_angles(start_deg, step_deg, end_deg);
-    if (n_ang < 1 || !is_pow2(Nx) || !is_pow2(Ny) || Nz < 1) return -1;
+    if (n_ang < 1 || Nx < 1 || Ny < 1 || Nz < 1) return -1;
     double k = orc_wavenumber(energy_eV);
     double *a = malloc(sizeof(double) * 2 * n_mat), *b = malloc(sizeof(double) * 2 * n_mat),
            *c = malloc(sizeof(double) * 2 * n_mat);
@@ -573,7 +594,7 @@ int orc_run_energy_linear(int Nx, int Ny, int Nz, int n_mat, double voxel,
 {
     const int64_t n_vox = (int64_t)Nx * Ny * Nz, n_pix = (int64_t)Nx * Ny;
     int n_ang = orc_num_angles(start_deg, step_deg, end_deg);
-    if (n_ang < 1 || !is_pow2(Nx) || !is_pow2(Ny) || Nz < 1) return -1;
+    if (n_ang < 1 || Nx < 1 || Ny < 1 || Nz < 1) return -1;
     double k = orc_wavenumber(energy_eV);
     double *a = malloc(sizeof(double) * 2 * n_mat), *b = malloc(sizeof(double) * 2 * n_mat),
            *c = malloc(sizeof(double) * 2 * n_mat);

@@ -568,6 +568,45 @@ def test_A14_any_Nz_definition_dft_along_z():
     assert np.array_equal(ca, cb) and np.allclose(a, b, rtol=1e-11, atol=1e-14 * a.max())
 
 
+def test_A14_any_Nx_Ny_definition_dft_along_x_and_y():
+    """Lateral sizes that are not powers of two (DESIGN.md 3-A14): the oracle takes the definition
+    of Eq. 6 along such an axis.  Pins, none of which calls the routine it checks: the brute-force 3-D DFT,
+    numpy's FFT (a library routine of the same definition), Parseval, a plane wave landing in exactly one bin with the
+    forward sign, and the whole pipeline: a uniform isotropic film of odd size puts everything into q = 0 with the
+    closed-form value, and linear mode equals definition mode on 12 x 10 x 3."""
+    rng = np.random.default_rng(6)
+    for shape in [(4, 6, 10), (3, 5, 7), (1, 12, 9), (2, 8, 6), (5, 4, 3)]:          # (Nz, Ny, Nx)
+        f = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+        F = oracle.fft3(f)
+        assert np.allclose(F, oracle.dft3_naive(f), rtol=0, atol=1e-11 * np.abs(F).max()), shape
+        assert np.allclose(F, np.fft.fftn(f), rtol=0, atol=1e-11 * np.abs(F).max()), shape
+        assert np.isclose((np.abs(F) ** 2).sum(), f.size * (np.abs(f) ** 2).sum(), rtol=1e-12)
+    ny, nx, my, mx = 6, 10, 2, 7
+    y = np.arange(ny).reshape(1, ny, 1); x = np.arange(nx).reshape(1, 1, nx)
+    f = np.exp(2j * np.pi * (my * y / ny + mx * x / nx)) * np.ones((3, ny, nx))
+    F = oracle.fft3(f)
+    G = F.copy(); G[0, my, mx] = 0
+    assert np.isclose(F[0, my, mx], 3 * ny * nx) and np.abs(G).max() < 1e-9
+    # uniform isotropic film, 9 x 15 x 1: I(q = 0) = k^4 N^2 |n^2 - 1|^2 / (16 pi^2), zero elsewhere (P2's closed form)
+    nx, ny = 15, 9
+    delta, beta, E = 1e-3, 5e-4, 285.0
+    mats = [(np.ones((1, ny, nx), np.float32), None, None, None)]
+    f1 = lambda v: np.array([[v]], np.float32)
+    w = W.Workload("film", nx, ny, 1, 5.0, mats, np.array([E]), f1(delta), f1(beta), f1(delta), f1(beta), (0.0, 0.0, 0.0),
+                   W.EWALD_NEAREST)                                             # one angle, 0 degrees: no interpolation
+    img, cnt = _run(w)
+    k = 2 * PI * E / 1239.84197
+    n2m1 = complex(-np.float32(delta), np.float32(beta)) * (complex(-np.float32(delta), np.float32(beta)) + 2.0)
+    expect = k ** 4 * (nx * ny) ** 2 * abs(n2m1) ** 2 / (16 * PI ** 2)
+    assert np.isclose(img[0, ny // 2, nx // 2], expect, rtol=1e-10)
+    rest = img[0].copy(); rest[ny // 2, nx // 2] = 0
+    assert rest.max() < 1e-18 * expect
+    w = W.tiny(seed=78, nx=12, ny=10, nz=3, n_mat=2, n_energy=1, voxel_nm=1.5, ewald=W.EWALD_TRILINEAR)
+    a, ca = _run(w)
+    b, cb = _run(w, linear=True)
+    assert np.array_equal(ca, cb) and np.allclose(a, b, rtol=1e-11, atol=1e-14 * a.max())
+
+
 # ================================================================ round-2 pins
 # Each of these ties one decision of the oracle, that no earlier pin reached, to a closed form written
 # out here from the paper's equations (none calls the oracle for its expected value).
