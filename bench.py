@@ -1,13 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the CyRSoXS hot path on B200 (contract: task prompt section 4).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg5]
 
 A "step" is one pass of the whole hot path (all energies x all E-field angles of the
 workload) over one synthetic morphology.  Metric: E-angle patterns/s (BASELINE.json), device
 timed with CUDA events on the launching stream; voxel.angle evaluations/s is reported beside
-it.  The default workload is BASELINE.json configs[1] (3-D cube 128^3, 10 energies x 36
-angles).  N > 1: energies are independent units, so every rank simulates its
+it.  BASELINE.json's metric names no config, so the default workload is the largest single-GPU one,
+configs[4] (1024 x 1024 x 512, 20 energies x 9 angles; configs[2] if the device or host is too small);
+the other configs are timed with fewer steps into the `per_config` key.  N > 1: energies are independent units, so every rank simulates its
 own slice of a N-times longer energy list on the same morphology -- no data-path collective,
 weak scaling.  `--impl reference` times the CPU oracle (as it stands) on the host cores.
 """
@@ -30,22 +31,6 @@ from paper_2209_13121_b200 import workloads as W  # noqa: E402
 
 METRIC = "E-angle patterns/s (device-timed)"
 UNIT = "patterns/s"
-
-# stages (cyrsoxs_stats) grouped by the kernel that runs them; the names are those of the SPECTRAL_BASIS
-# kernels the default run launches (PER_ENERGY: k_xpass_chi / k_ewald_chi in the first and third slot)
-STAGES_OF_KERNEL = {"k_xbasis2 (fields + FFT along x)": ["xpass"], "k_col2p (FFT along z, then along y)": ["zpass", "ypass"],
-                    "k_ewald_basis (Ewald gather)": ["ewald"], "k_rotate_avg (rotate back + average)": ["rotate"]}
-# what bounds each kernel: the FFT passes stream HBM; the two image kernels do not
-LIMITER = {"k_xbasis2 (fields + FFT along x)": "HBM stream, instruction-issue limited (~280-600 instr/voxel, DESIGN 7.1)",
-           "k_col2p (FFT along z, then along y)": "HBM stream",
-           "k_ewald_basis (Ewald gather)": "instruction issue + L2 gather latency, not HBM (DESIGN 7.3)",
-           "k_rotate_avg (rotate back + average)": "L1 data-pipe wavefronts / latency of the bilinear gathers, not HBM (DESIGN 7.4)"}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch (average over the kernel's launches of a step) from the
-# committed ncu --set full capture profiles/r1e_cfg2_ncu_summary.md; ncu flushes the caches before each replay and
-# part of the writes is still in L2 when a kernel ends, so this can be below the algorithmic bytes
-NCU_TRAFFIC = {("cfg2", "k_xbasis2 (fields + FFT along x)"): 59.7e6, ("cfg2", "k_col2p (FFT along z, then along y)"): 75.6e6,
-               ("cfg2", "k_ewald_basis (Ewald gather)"): 11.6e6, ("cfg2", "k_rotate_avg (rotate back + average)"): 2.4e6}
-
 
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -148,44 +133,69 @@ class ClockSampler(threading.Thread):
 
 
 def oracle_sample(w, budget_s: float = 20.0):
-    """The oracle as it stands (definition mode: per angle polarization, three FFTs, Ewald,
-    rotate) on a bounded sample of the workload: as many of its angles as fit the budget for the
-    first energy and, if all of them fit, as many further energies as fit (at most all).
-    Returns (patterns/s, n_energies, n_angles, seconds, threads)."""
+    """The oracle as it stands (definition mode: per angle polarization, three FFTs, Ewald, rotate) on a bounded
+    sample of the workload that takes about `budget_s` seconds: the first `planes` z planes of the morphology (all of
+    them if one full-size angle fits the budget), as many of the workload's angles as fit for the first energy and, if
+    all of them fit, as many further energies as fit.  A sample thinner than the workload is scaled to the full size by
+    its voxel.angle rate (the paper reports wall time O(N) in the number of voxels).
+    Returns (patterns/s of the full-size workload, description, seconds, threads)."""
     import oracle
 
-    def run(n_e, n_a):
+    def run(planes, n_e, n_a):
+        mats = [tuple(None if a is None else a[:planes] for a in m) for m in w.materials]
         t0 = time.perf_counter()
-        oracle.run(w.materials, w.voxel_nm, w.energies[:n_e], w.delta_par[:n_e], w.beta_par[:n_e], w.delta_perp[:n_e],
+        oracle.run(mats, w.voxel_nm, w.energies[:n_e], w.delta_par[:n_e], w.beta_par[:n_e], w.delta_perp[:n_e],
                    w.beta_perp[:n_e], (w.angles[0], w.angles[1], w.angles[0] + (n_a - 1) * w.angles[1]), w.ewald)
         return time.perf_counter() - t0
 
-    t1 = run(1, 1)                                           # also warms the page cache / thread pool
-    n_a = int(max(1, min(w.n_angles, budget_s / max(t1, 1e-9))))
-    n_e = 1
-    if n_a == w.n_angles:
-        n_e = int(max(1, min(w.n_energy, budget_s / max(t1 * n_a, 1e-9))))
-    dt = run(n_e, n_a)
-    return n_e * n_a / dt, n_e, n_a, dt, oracle.num_threads()
+    p0 = min(w.Nz, 2)
+    run(p0, 1, 1)                                            # warms the page cache / thread pool
+    t0 = run(p0, 1, 1)
+    planes = p0
+    while planes * 2 <= w.Nz and t0 * (planes * 2 / p0) * 1.3 <= budget_s:      # 1.3: the FFT's log factor and cache effects
+        planes *= 2
+    if planes * 2 > w.Nz and t0 * (w.Nz / p0) * 1.3 <= budget_s:
+        planes = w.Nz
+    t1 = t0 * planes / p0 * (1.3 if planes > p0 else 1.0)
+    n_a = int(max(1, min(w.n_angles, budget_s / max(t1, 1e-9)))) if planes == w.Nz else 1
+    n_e = int(max(1, min(w.n_energy, budget_s / max(t1 * n_a, 1e-9)))) if n_a == w.n_angles else 1
+    dt = run(planes, n_e, n_a)
+    vox_angle_per_s = float(planes) * w.Ny * w.Nx * n_e * n_a / dt
+    desc = (f"{n_e} of {w.n_energy} energies x {n_a} of {w.n_angles} angles on {planes} of {w.Nz} z planes of the same morphology, "
+            f"definition mode (polarization, 3 FFTs, Ewald, rotate per angle), {dt:.1f} s"
+            + ("" if planes == w.Nz else "; scaled to the full depth by voxel.angle/s (wall time O(N), PAPER.md:473)"))
+    return vox_angle_per_s / w.n_vox, desc, dt, oracle.num_threads()
+
+
+def resolve_workload(name: str) -> str:
+    if name != "auto":
+        return name
+    try:
+        import torch
+        if torch.cuda.is_available():
+            return pick_default_workload(torch.device("cuda", 0))
+    except Exception:
+        pass
+    return "cfg3"
 
 
 def run_reference(args, rank, world):
     if rank != 0:
         return
-    w = make_workload(args.workload, 0, 1)
+    name = resolve_workload(args.workload)
+    w = make_workload(name, 0, 1)
     vals = []
     for i in range(args.warmup + args.steps):
-        v, ne, na, dt, cores = oracle_sample(w, budget_s=max(2.0, 60.0 / (args.warmup + args.steps)))
+        v, desc, dt, cores = oracle_sample(w, budget_s=max(1.0, 90.0 / (args.warmup + args.steps)))
         if i >= args.warmup:
-            vals.append((v, ne * na, dt, ne, na))
-    value = sum(v[1] for v in vals) / sum(v[2] for v in vals)
-    sample = (f"{vals[0][3]} of {w.n_energy} energies x {vals[0][4]} of {w.n_angles} angles per step, definition mode "
-              "(polarization, 3 FFTs, Ewald, rotate per angle)")
+            vals.append((v, dt, desc))
+    value = sum(v[0] * v[1] for v in vals) / sum(v[1] for v in vals)          # time-weighted mean rate
+    sample = vals[0][2] + " per step"
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * sum(v[2] for v in vals) / len(vals), "higher_is_better": True,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sum(v[1] for v in vals) / len(vals), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_label(w, args.workload), "sample": sample},
+        "config": {"workload": workload_label(w, name), "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -193,26 +203,45 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def run_ours(args, rank, world, local_rank):
+def kernel_groups(st):
+    """Stages (cyrsoxs_stats) grouped by the kernel that runs them, with what bounds each kernel.  The
+    names are those of the SPECTRAL_BASIS kernels the default run launches."""
+    g = {"k_xbasis3 (fields + FFT along x)": (["xpass"], "HBM stream, instruction-issue limited (DESIGN 7.1)"),
+         "k_col2p (FFT along z, then along y)": (["zpass", "ypass"], "HBM stream")}
+    g["k_ewald_basis (Ewald gather)"] = (["ewald"], "instruction issue + L2 gather latency, not HBM (DESIGN 7.3)")
+    g["k_rotate_avg (rotate back + average)"] = (["rotate"], "L1 data-pipe wavefronts / latency of the bilinear gathers, not HBM (DESIGN 7.4)")
+    return g
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, from the tracked ncu captures
+    listed in profiles/ncu_traffic.json (each entry names its capture file and the commit it was taken at)."""
+    try:
+        tab = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+    except Exception:
+        return None, None
+    short = kernel.split(" ")[0]
+    ent = tab.get(workload, {}).get(short)
+    if not ent:
+        return None, None
+    return float(ent["dram_bytes_per_launch"]), {k: ent[k] for k in ("capture", "commit") if k in ent}
+
+
+def measure(name, args, rank, world, dev, steps, warmup, with_e2e, with_clocks, alg, streamed=0):
+    """Device-timed steps of one workload (+ per-stage pass, + e2e through host buffers).  Returns a dict."""
     import torch
     import torch.distributed as dist
-    from paper_2209_13121_b200 import binding, build
-    build.build()
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-
-    w = make_workload(args.workload, rank, world)
-    alg = {"auto": binding.ALG_AUTO, "per_energy": binding.ALG_PER_ENERGY, "spectral": binding.ALG_SPECTRAL_BASIS}[args.alg]
+    from paper_2209_13121_b200 import binding
+    w = make_workload(name, rank, world)
+    local_rank = dev.index
     mats = [tuple(None if a is None else torch.from_numpy(a).to(dev) for a in m) for m in w.materials]
     ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
-    if args.streamed > 0:
+    if streamed > 0:
         # memory-minimising mode (DESIGN.md 12): the morphology stays in pinned host memory and is streamed
         # through the device group by group at every run -- PCIe traffic is then inside every timed step
         del mats
         pinned_main = [tuple(None if a is None else torch.from_numpy(a).pin_memory() for a in m) for m in w.materials]
-        ctx.set_morphology_streamed(pinned_main, args.streamed)
+        ctx.set_morphology_streamed(pinned_main, streamed)
     else:
         ctx.set_morphology(mats)
     ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
@@ -235,95 +264,154 @@ def run_ours(args, rank, world, local_rank):
         b.record(stream)
         return a, b
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         one_step()
     barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    evs = [one_step() for _ in range(args.steps)]
-    if sampler.nvml is not None:
+    sampler = ClockSampler(local_rank) if with_clocks else None
+    if sampler:
+        sampler.start()
+    evs = [one_step() for _ in range(steps)]
+    if sampler and sampler.nvml is not None:
         sampler.sample_once()                           # at least one sample while the queue is still draining
     barrier()
-    sampler.stop_flag = True
-    sampler.join(timeout=3)
-    step_ms = [a.elapsed_time(b) for a, b in evs]
-    total_ms = float(sum(step_ms))
+    if sampler:
+        sampler.stop_flag = True
+        sampler.join(timeout=3)
+    total_ms = float(sum(a.elapsed_time(b) for a, b in evs))
     if world > 1:
         t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
     st = ctx.stats()
-    launches = st["kernel_launches"] * args.steps
-
-    # ---- end to end through the C ABI with host buffers (H2D + D2H inside the timed region)
-    pinned = [tuple(None if a is None else torch.from_numpy(a).pin_memory() for a in m) for m in w.materials]
-    h_out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32).pin_memory()
-    ctx2 = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
-    ctx2.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
-    ctx2.set_angles(*w.angles); ctx2.set_ewald(w.ewald); ctx2.set_algorithm(alg)
-    h2d = sum(a.numel() * 4 for m in pinned for a in m if a is not None)
-    d2h = h_out.numel() * 4
-
-    def e2e_step():
-        flush.fill_(1)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        ctx2.set_morphology_host(pinned, sptr)
-        ctx2.run(h_out.data_ptr(), sptr)
-        b.record(stream)
-        return a, b
-
-    for _ in range(max(1, min(args.warmup, 3))):
-        e2e_step()
-    barrier()
-    n_e2e = max(1, min(args.steps, 10))
-    ev2 = [e2e_step() for _ in range(n_e2e)]
-    barrier()
-    e2e_all = sorted(a.elapsed_time(b) for a, b in ev2)
-    e2e_ms = float(sum(e2e_all)) / n_e2e
-    e2e_median_ms = float(e2e_all[len(e2e_all) // 2])
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    res = {"w": w, "ms_per_step": total_ms / steps, "total_ms": total_ms, "launches_per_step": int(st["kernel_launches"]), "st": st,
+           "clocks": sampler.summary() if sampler else None}
+    if args.quick:
+        return res
 
     # ---- per-stage device times (CUDA events on the run's stream, inside the library) for the roofline
     ctx.set_profiling(True)
     stage_ms = {k: 0.0 for k in binding.STAGES}
-    nprof = max(1, min(args.steps, 5))
+    nprof = max(1, min(steps, 5))
     for _ in range(nprof):
         flush.fill_(1)
         ctx.run(out.data_ptr(), sptr)
         s2 = ctx.stats()
         for k in stage_ms:
-            stage_ms[k] += s2["stage_ms"][k]
+            stage_ms[k] += s2["stage_ms"][k] / nprof
     ctx.set_profiling(False)
-    # the dominant KERNEL: stages are grouped by the kernel that runs them (the z and y passes are two
-    # launches of the same column-pass kernel), largest summed device time wins
-    ktime = {k: sum(stage_ms[s_] for s_ in v) for k, v in STAGES_OF_KERNEL.items()}
+    res["stage_ms"] = stage_ms
+
+    # ---- end to end through the C ABI with host buffers (H2D + D2H inside the timed region)
+    if with_e2e:
+        pinned = [tuple(None if a is None else torch.from_numpy(a).pin_memory() for a in m) for m in w.materials]
+        h_out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32).pin_memory()
+        del ctx, mats                                   # the e2e context owns its own device copy of the morphology
+        ctx2 = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+        ctx2.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+        ctx2.set_angles(*w.angles); ctx2.set_ewald(w.ewald); ctx2.set_algorithm(alg)
+
+        def e2e_step():
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            ctx2.set_morphology_host(pinned, sptr)
+            ctx2.run(h_out.data_ptr(), sptr)
+            b.record(stream)
+            return a, b
+
+        for _ in range(max(1, min(warmup, 3))):
+            e2e_step()
+        barrier()
+        n_e2e = max(1, min(steps, 10))
+        ev2 = [e2e_step() for _ in range(n_e2e)]
+        barrier()
+        e2e_all = sorted(a.elapsed_time(b) for a, b in ev2)
+        e2e_ms = float(sum(e2e_all)) / n_e2e
+        if world > 1:
+            t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_ms = float(t.item())
+        res["e2e"] = {"ms": e2e_ms, "median_ms": float(e2e_all[len(e2e_all) // 2]),
+                      "h2d": sum(a.numel() * 4 for m in pinned for a in m if a is not None), "d2h": h_out.numel() * 4}
+        del ctx2, pinned, h_out
+    torch.cuda.empty_cache()
+    return res
+
+
+def roofline_of(name, res, peak, peak_src):
+    """The roofline object of one measured workload: the kernel with the largest summed device time."""
+    w, st, stage_ms = res["w"], res["st"], res["stage_ms"]
+    groups = kernel_groups(st)
+    ktime = {k: sum(stage_ms[s_] for s_ in v[0]) for k, v in groups.items()}
     dom = max(ktime, key=lambda k: ktime[k])
-    dom_stages = STAGES_OF_KERNEL[dom]
-    peak, peak_src = load_peaks()
+    dom_stages = groups[dom][0]
     dom_launches = max(1, sum(st["stage_launches"][s_] for s_ in dom_stages))
-    dom_ms_per_launch = ktime[dom] / nprof / dom_launches
+    dom_ms_per_launch = ktime[dom] / dom_launches
     dom_bytes_per_launch = sum(st["stage_bytes"][s_] for s_ in dom_stages) / dom_launches
     achieved = dom_bytes_per_launch / (dom_ms_per_launch * 1e-3) / 1e9 if dom_ms_per_launch > 0 else 0.0
     whole_bytes = sum(st["stage_bytes"].values())
+    ms = res["ms_per_step"]
     # SURVEY.md 8(d) contract model M0: (16 c + 96) bytes per voxel per energy (+28 per pixel in 2-D)
     m0_bytes = w.n_energy * ((16.0 * w.n_mat + 96.0) * w.n_vox + (28.0 * w.Nx * w.Ny if w.Nz == 1 else 0.0))
+    traffic, traffic_src = ncu_traffic(name, dom)
+    return {"bound": "hbm", "kernel": dom, "stages": dom_stages, "launches_per_step": dom_launches,
+            "share_of_step": ktime[dom] / max(sum(ktime.values()), 1e-12),
+            "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_vs_nominal_8000": achieved / 8000.0,
+            "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src, "limiter": groups[dom][1],
+            "bytes_per_launch": dom_bytes_per_launch, "ms_per_launch": dom_ms_per_launch,
+            "stage_ms_per_step": stage_ms,
+            "stage_gbs": {k: (st["stage_bytes"][k] / (stage_ms[k] * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0) for k in stage_ms},
+            "whole_step": {"bytes": whole_bytes, "achieved": whole_bytes / (ms * 1e-3) / 1e9, "frac": whole_bytes / (ms * 1e-3) / 1e9 / peak},
+            "whole_step_vs_M0": {"bytes": m0_bytes, "achieved": m0_bytes / (ms * 1e-3) / 1e9, "frac": m0_bytes / (ms * 1e-3) / 1e9 / peak,
+                                 "note": "M0 = (16c+96) B/voxel/energy (SURVEY 8(d)); this build moves fewer bytes "
+                                         "(energy-independent spectra, pruned windows), so frac > 1 is possible"}}
+
+
+def pick_default_workload(dev) -> str:
+    """BASELINE.json names no config for the metric: the headline is the largest single-GPU one, configs[4]
+    (1024 x 1024 x 512; 17 GB of morphology, 11 GB of workspace, 17 GB pinned for e2e).  A smaller device or
+    host falls back to configs[2] and says so in config.workload."""
+    import torch
+    try:
+        free_b, _ = torch.cuda.mem_get_info(dev)
+        host_gb = os.sysconf("SC_PAGE_SIZE") * os.sysconf("SC_PHYS_PAGES") / 2**30
+        return "cfg5" if free_b >= 60 * 2**30 and host_gb >= 100 else "cfg3"
+    except Exception:
+        return "cfg3"
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2209_13121_b200 import binding, build
+    build.build()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    alg = {"auto": binding.ALG_AUTO, "per_energy": binding.ALG_PER_ENERGY, "spectral": binding.ALG_SPECTRAL_BASIS}[args.alg]
+    name = resolve_workload(args.workload)
+    fallback = " [fallback: configs[4] does not fit this device/host]" if args.workload == "auto" and name != "cfg5" else ""
+    res = measure(name, args, rank, world, dev, args.steps, args.warmup, with_e2e=True, with_clocks=True, alg=alg, streamed=args.streamed)
+    w, st = res["w"], res["st"]
+    if args.quick:
+        if rank == 0:
+            print(json.dumps({"quick": True, "workload": name, "ms_per_step": res["ms_per_step"], "launches_per_step": res["launches_per_step"]}), flush=True)
+        return
+    peak, peak_src = load_peaks()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-
-    patterns = w.n_energy * w.n_angles * world * args.steps
-    value = patterns / (total_ms * 1e-3)
+    patterns = w.n_energy * w.n_angles * world
+    value = patterns / (res["ms_per_step"] * 1e-3)
+    e2e = res["e2e"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {
-            "workload": workload_label(w, args.workload),
+            "workload": workload_label(w, name) + fallback,
             "algorithm": {1: "per_energy", 2: "spectral_basis"}.get(st["algorithm"], "?"),
             "energy_batch": st["energy_batch"], "l2": "flushed between timed steps (256 MB write)",
             "parallelism": f"energies sharded over {world} GPU(s), no collective",
@@ -333,33 +421,33 @@ def run_ours(args, rank, world, local_rank):
         "voxel_angle_evals_per_s": value * w.n_vox,
         "device_bytes": {"morphology": int(sum(a.nbytes for m in w.materials for a in m if a is not None)) if args.streamed == 0 else 0,
                          "workspace": int(st["workspace_bytes"])},
-        "e2e": {"value": w.n_energy * w.n_angles * world / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "ms_per_step_median": e2e_median_ms,
+        "e2e": {"value": patterns / (e2e["ms"] * 1e-3), "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"],
+                "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": e2e["ms"], "ms_per_step_median": e2e["median_ms"],
                 "note": "PCIe-bound: uploads the whole morphology every step"},
-        "gpu_launches": int(launches),
-        "clocks": sampler.summary(),
-        "roofline": {"bound": "hbm", "kernel": dom, "stages": dom_stages, "launches_per_step": dom_launches,
-                     "share_of_step": ktime[dom] / max(sum(ktime.values()), 1e-12),
-                     "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "frac_vs_nominal_8000": achieved / 8000.0,
-                     "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
-                     "limiter": LIMITER[dom],
-                     "bytes_per_launch": dom_bytes_per_launch, "ms_per_launch": dom_ms_per_launch,
-                     "stage_ms_per_step": {k: v / nprof for k, v in stage_ms.items()},
-                     "stage_gbs": {k: (st["stage_bytes"][k] / (stage_ms[k] / nprof * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0)
-                                   for k in stage_ms},
-                     "whole_step": {"bytes": whole_bytes, "achieved": whole_bytes / (total_ms / args.steps * 1e-3) / 1e9,
-                                    "frac": whole_bytes / (total_ms / args.steps * 1e-3) / 1e9 / peak},
-                     "whole_step_vs_M0": {"bytes": m0_bytes, "achieved": m0_bytes / (total_ms / args.steps * 1e-3) / 1e9,
-                                          "frac": m0_bytes / (total_ms / args.steps * 1e-3) / 1e9 / peak,
-                                          "note": "M0 = (16c+96) B/voxel/energy (SURVEY 8(d)); this build moves fewer bytes "
-                                                  "(energy-independent spectra, pruned windows), so frac > 1 is possible"}},
+        "gpu_launches": int(res["launches_per_step"] * args.steps),
+        "clocks": res["clocks"],
+        "roofline": roofline_of(name, res, peak, peak_src),
     }
     if world == 1 and not args.no_cpu_baseline:
-        v, ne, na, dt, cores = oracle_sample(w, budget_s=20.0)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"{ne} of {w.n_energy} energies x {na} of {w.n_angles} angles of the same workload, "
-                                          f"definition mode, {dt:.1f} s"}
+        v, desc, dt, cores = oracle_sample(w, budget_s=20.0)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    del res, w
+    if world == 1 and not args.no_per_config:
+        # the other BASELINE.json configs, measured the same way with fewer steps (no e2e, no CPU baseline)
+        per = {}
+        for other in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5"):
+            if other == name or (other == "cfg5" and name != "cfg5"):
+                continue
+            r = measure(other, args, 0, 1, dev, 5, 3, with_e2e=False, with_clocks=False, alg=alg)
+            rf = roofline_of(other, r, peak, peak_src)
+            wo = r["w"]
+            per[other] = {"workload": workload_label(wo, other), "ms_per_step": r["ms_per_step"],
+                          "patterns_per_s": wo.n_energy * wo.n_angles / (r["ms_per_step"] * 1e-3),
+                          "dominant_kernel": rf["kernel"], "frac": rf["frac"], "traffic": rf["traffic"],
+                          "stage_ms_per_step": rf["stage_ms_per_step"],
+                          "whole_step_frac": rf["whole_step"]["frac"], "whole_step_vs_M0_frac": rf["whole_step_vs_M0"]["frac"]}
+            del r, wo
+        line["per_config"] = per
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -371,9 +459,11 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--workload", default="auto", help="cfg1 .. cfg5; auto: cfg5 (BASELINE.json configs[4]), cfg3 if it does not fit")
     ap.add_argument("--alg", default="auto", choices=["auto", "per_energy", "spectral"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config key (the other BASELINE.json configs)")
+    ap.add_argument("--quick", action="store_true", help="device-timed steps only (no e2e, no per-stage pass, no CPU baseline): the command ncu wraps")
     ap.add_argument("--streamed", type=int, default=0, help="materials per group of cyrsoxs_set_morphology_streamed (0: resident)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -87,10 +87,13 @@ typedef struct {
 } cyrsoxs_stats;
 
 /* Creates a context for an Nx x Ny x Nz voxel model with n_mat materials and cubic voxels of
- * edge voxel_nm ("voxels are considered perfect cubes").  Nx and Ny must be powers of two,
- * 4 <= Nx <= 2048, 2 <= Ny <= 2048; Nz is a power of two up to 2048 or any length up to 512 (the
- * paper uses Nz = 63; such a z axis is transformed by a pruned direct DFT); 1 <= n_mat <= 32,
- * voxel_nm > 0 (else INVALID_ARG).  Uses the current CUDA device.  *out is NULL on failure. */
+ * edge voxel_nm ("voxels are considered perfect cubes").  4 <= Nx <= 2048, 2 <= Ny <= 2048,
+ * 1 <= Nz <= 2048.  Powers of two take the FFT kernels (the paper recommends them laterally); an
+ * axis of any other length (the paper uses Nz = 63) is transformed by the definition of Eq. 6
+ * evaluated at the bins the Ewald step can reach (a pruned direct DFT, O(N W) per line: a functional
+ * path for thin films and odd lateral sizes, not a tuned FFT).  Nx that is not a power of two needs
+ * CYRSOXS_ALG_SPECTRAL_BASIS (AUTO picks it; PER_ENERGY returns NOT_IMPLEMENTED at run).
+ * 1 <= n_mat <= 32, voxel_nm > 0 (else INVALID_ARG).  Uses the current CUDA device.  *out is NULL on failure. */
 cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm, cyrsoxs_ctx **out);
 
 /* Morphology (memory model P:199-203): for each material m four DEVICE arrays of

@@ -27,7 +27,7 @@ constexpr double kPi = 3.141592653589793;
 constexpr double kHcEvNm = 1239.84197;
 constexpr int kMaxAngles = 4096;
 constexpr int kMaxLog2 = 11;
-constexpr int kMaxNzAny = 512;         // longest z axis that is not a power of two (direct DFT pass)
+constexpr int kMaxAny = 2048;           // longest axis that is not a power of two (direct DFT passes)
 
 struct DevBuf {
     void *p = nullptr;
@@ -78,7 +78,7 @@ struct cyrsoxs_ctx {
     // SPECTRAL_BASIS plan (rebuilt per run from the morphology's NULL pattern and the optics)
     int n_pack = 0;
     std::vector<int> basis_kind, basis_mat;     // [2 n_pack]
-    DevBuf d_bcoef, d_bkind;
+    DevBuf d_bcoef, d_bkind, d_bmat;
     bool plan_dirty = true;
     unsigned long long null_pattern = ~0ull;
     // workspace
@@ -322,13 +322,19 @@ template <int LOGN, int PW> cyrsoxs_status launch_colpass_pair_t(cyrsoxs_ctx *c,
 cyrsoxs_status launch_colpass(cyrsoxs_ctx *c, cudaStream_t st, int N, const ColParams &p, int n_lo, int n_hi, int pitch)
 {
     if (!is_pow2(N)) {
-        // a z axis of any length (DESIGN 3-A14): the pruned direct DFT
-        const size_t smem = sizeof(float2) * ((size_t)N * DFT_TX + N);
-        if (cyrsoxs_status a = allow_smem(c, k_coldft, sizeof(float2) * ((size_t)kMaxNzAny * DFT_TX + kMaxNzAny))) return a;
+        // an axis of any length (DESIGN 3-A14): the pruned direct DFT
+        const int tx = dft_tx(N);
+        const size_t smem = sizeof(float2) * ((size_t)N * tx + N);
         ColParams q = p;
-        q.n_tiles = pitch / DFT_TX;
+        q.n_tiles = pitch / tx;
         dim3 grid((unsigned)(q.n_tiles * n_lo), (unsigned)n_hi);
-        k_coldft<<<grid, DFT_TX * DFT_OG, smem, st>>>(q, N);
+        if (tx == 32) {
+            if (cyrsoxs_status a = allow_smem(c, k_coldft<32>, sizeof(float2) * ((size_t)512 * 32 + 512))) return a;
+            k_coldft<32><<<grid, DFT_THREADS, smem, st>>>(q, N);
+        } else {
+            if (cyrsoxs_status a = allow_smem(c, k_coldft<8>, sizeof(float2) * ((size_t)kMaxAny * 8 + kMaxAny))) return a;
+            k_coldft<8><<<grid, DFT_THREADS, smem, st>>>(q, N);
+        }
         CUDA_TRY(c, cudaGetLastError());
         return CYRSOXS_OK;
     }
@@ -523,22 +529,24 @@ cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int
     return launch_rotate(c, st, e0, eb, d_out, d_cnt);
 }
 
-template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch)
+// rows: rows (of Nx voxels) this launch transforms, starting at the morphology pointers of `mp`; fstride: distance
+// (float2 elements) between the packs of `out`.
+template <int LOGN> cyrsoxs_status launch_xbasis_t(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch,
+                                                   int rows, size_t fstride)
 {
     using Cfg = XB2Cfg<LOGN>;
     if (cyrsoxs_status a = allow_smem(c, k_xbasis2<LOGN>, Cfg::SMEM)) return a;
-    const int rows = c->Ny * c->Nz;
     dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS);
-    k_xbasis2<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(mp, out, rows, wx, pitch, (const float2 *)c->twx.p);
+    k_xbasis2<LOGN><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(mp, out, rows, fstride, wx, pitch, (const float2 *)c->twx.p);
     CUDA_TRY(c, cudaGetLastError());
     return CYRSOXS_OK;
 }
 
-template <int LOGN> cyrsoxs_status launch_xbasis3_t(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch)
+template <int LOGN> cyrsoxs_status launch_xbasis3_t(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch,
+                                                    int rows, size_t fstride)
 {
     using Cfg = XB3Cfg<LOGN>;
     if (cyrsoxs_status a = allow_smem(c, k_xbasis3<LOGN>, Cfg::SMEM)) return a;
-    const int rows = c->Ny * c->Nz;
     dim3 grid((rows + Cfg::ROWS - 1) / Cfg::ROWS);
     size_t smem = Cfg::SMEM;
 #ifdef CYRSOXS_TUNING          // sweep aid, compiled out of the shipped library: occupancy sensitivity
@@ -548,18 +556,29 @@ template <int LOGN> cyrsoxs_status launch_xbasis3_t(cyrsoxs_ctx *c, cudaStream_t
 #ifdef CYRSOXS_TUNING
     if (const char *e = getenv("CYRSOXS_XB3_AHEAD")) ahead = atoi(e);
 #endif
-    k_xbasis3<LOGN><<<grid, Cfg::THREADS, smem, st>>>(mp, out, rows, (size_t)rows * pitch, wx, pitch, (const float2 *)c->tw2x.p, ahead);
+    k_xbasis3<LOGN><<<grid, Cfg::THREADS, smem, st>>>(mp, out, rows, fstride, wx, pitch, (const float2 *)c->tw2x.p, ahead);
     CUDA_TRY(c, cudaGetLastError());
     return CYRSOXS_OK;
 }
 
-cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch)
+// pack0 / mat0: first pack and first material of `mp` in the basis plan (non-zero for the material groups of the streamed mode)
+cyrsoxs_status launch_xbasis(cyrsoxs_ctx *c, cudaStream_t st, const MorphPtrs &mp, float2 *out, const Window &wx, int pitch,
+                             int rows, size_t fstride, int pack0 = 0, int mat0 = 0, int n_pack = -1)
 {
+    if (!is_pow2(c->Nx)) {
+        // a row length that is not a power of two: direct DFT at the window's bins (k_xdft)
+        const size_t smem = sizeof(float2) * 2 * (size_t)c->Nx;
+        if (n_pack < 0) n_pack = c->n_pack;
+        k_xdft<<<rows, XDFT_THREADS, smem, st>>>(mp, (const int *)c->d_bkind.p + 2 * pack0, (const int *)c->d_bmat.p + 2 * pack0, mat0, n_pack, out,
+                                                 rows, fstride, wx, pitch, (const float2 *)c->twx.p, c->Nx);
+        CUDA_TRY(c, cudaGetLastError());
+        return CYRSOXS_OK;
+    }
     switch (ilog2(c->Nx)) {
-#define CASE3(L) case L: return launch_xbasis3_t<L>(c, st, mp, out, wx, pitch);
+#define CASE3(L) case L: return launch_xbasis3_t<L>(c, st, mp, out, wx, pitch, rows, fstride);
         CASE3(6) CASE3(7) CASE3(8) CASE3(9) CASE3(10) CASE3(11)
 #undef CASE3
-#define CASE(L) case L: return launch_xbasis_t<L>(c, st, mp, out, wx, pitch);
+#define CASE(L) case L: return launch_xbasis_t<L>(c, st, mp, out, wx, pitch, rows, fstride);
         CASE(2) CASE(3) CASE(4) CASE(5)
 #undef CASE
     }
@@ -629,9 +648,11 @@ cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c, cudaStream_t st)
     cyrsoxs_status s;
     if ((s = ensure(c, c->d_bcoef, sizeof(float2) * coef.size())) != CYRSOXS_OK) return s;
     if ((s = ensure(c, c->d_bkind, sizeof(int) * nb)) != CYRSOXS_OK) return s;
+    if ((s = ensure(c, c->d_bmat, sizeof(int) * nb)) != CYRSOXS_OK) return s;
     // pageable sources: staged by the driver before these calls return; ordered after the stream's earlier work
     CUDA_TRY(c, cudaMemcpyAsync(c->d_bcoef.p, coef.data(), sizeof(float2) * coef.size(), cudaMemcpyHostToDevice, st));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_bkind.p, c->basis_kind.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_bmat.p, c->basis_mat.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
     c->plan_dirty = false;
     return CYRSOXS_OK;
 }
@@ -648,7 +669,7 @@ cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &
     for (int m = 0; m < c->n_mat; ++m) (is_aligned(c, m) ? n_al : n_iso) += 1;
     if (!c->streamed) {
         StageTimer t(c, st, CYRSOXS_STAGE_XPASS);
-        if ((s = launch_xbasis(c, st, c->mp, A1, wx, pitch)) != CYRSOXS_OK) return s;
+        if ((s = launch_xbasis(c, st, c->mp, A1, wx, pitch, (int)rows, rows * (size_t)pitch)) != CYRSOXS_OK) return s;
     } else {
         // Memory-minimising mode (the paper's Algorithm 2/3 idea): material groups are
         // uploaded into a double-buffered staging area on the copy stream while the previous group's
@@ -687,7 +708,7 @@ cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &
             CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_stage_ready[slot], 0));
             {
                 StageTimer t(c, st, CYRSOXS_STAGE_XPASS);
-                if ((s = launch_xbasis(c, st, sub, A1 + (size_t)pack0 * fstride, wx, pitch)) != CYRSOXS_OK) return s;
+                if ((s = launch_xbasis(c, st, sub, A1 + (size_t)pack0 * fstride, wx, pitch, (int)rows, fstride, pack0, m0, (fields + 1) / 2)) != CYRSOXS_OK) return s;
             }
             CUDA_TRY(c, cudaEventRecord(c->ev_stage_free[slot], st));
             pack0 += (fields + 1) / 2;
@@ -774,9 +795,8 @@ cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm,
     if (!out) return CYRSOXS_ERR_INVALID_ARG;
     *out = nullptr;
     const int maxn = 1 << kMaxLog2;
-    if (!is_pow2(Nx) || !is_pow2(Ny) || Nx < 4 || Ny < 2 || Nz < 1 || Nx > maxn || Ny > maxn || Nz > maxn)
-        return CYRSOXS_ERR_INVALID_ARG;
-    if (!is_pow2(Nz) && Nz > kMaxNzAny) return CYRSOXS_ERR_INVALID_ARG;      // DESIGN 3-A14
+    static_assert(kMaxAny <= (1 << kMaxLog2), "direct-DFT passes cover every accepted length");
+    if (Nx < 4 || Ny < 2 || Nz < 1 || Nx > maxn || Ny > maxn || Nz > maxn) return CYRSOXS_ERR_INVALID_ARG;      // DESIGN 3-A14
     if (n_mat < 1 || n_mat > MAX_MAT || !(voxel_nm > 0.f) || !isfinite(voxel_nm)) return CYRSOXS_ERR_INVALID_ARG;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CYRSOXS_ERR_CUDA; }
@@ -807,7 +827,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
     clear_prof(c);
     for (void *p : c->owned_morph) cudaFree(p);
     for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->d_tiles[4], &c->d_tiles[5], &c->d_tiles[6], &c->d_tiles[7], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz, &c->tw2x, &c->tw2y, &c->tw2z,
-                      &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind, &c->red})
+                      &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind, &c->d_bmat, &c->red})
         release(*b);
     release(c->stage_morph[0]); release(c->stage_morph[1]);
     for (int i = 0; i < 2; ++i) {
@@ -1156,7 +1176,10 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     // (register-first x pass, real fields) costs about half of a PER_ENERGY one (measured on cfg3: 0.31 ms
     // per pack against 0.6 ms per field), hence the factor 2
     int alg = c->alg;
-    if (alg == CYRSOXS_ALG_AUTO) alg = (c->streamed || 2 * NCHI * c->nE >= c->n_pack) ? CYRSOXS_ALG_SPECTRAL_BASIS : CYRSOXS_ALG_PER_ENERGY;
+    if (alg == CYRSOXS_ALG_AUTO)
+        alg = (c->streamed || !is_pow2(c->Nx) || 2 * NCHI * c->nE >= c->n_pack) ? CYRSOXS_ALG_SPECTRAL_BASIS : CYRSOXS_ALG_PER_ENERGY;
+    if (!is_pow2(c->Nx) && alg != CYRSOXS_ALG_SPECTRAL_BASIS)
+        return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "Nx that is not a power of two needs CYRSOXS_ALG_SPECTRAL_BASIS (or AUTO)");
     if (c->streamed && alg != CYRSOXS_ALG_SPECTRAL_BASIS)
         return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "a streamed morphology needs CYRSOXS_ALG_SPECTRAL_BASIS (or AUTO)");
     const bool spectral = alg == CYRSOXS_ALG_SPECTRAL_BASIS;

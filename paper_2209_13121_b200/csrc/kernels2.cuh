@@ -140,39 +140,50 @@ k_col2p(const ColParams p)
 
 // Strided pass for a length that is not a power of two (the z axis only: the paper uses Nz = 63,
 // P:459): the definition of Eq. 6 evaluated directly, and only at the window's bins -- the "direct DFT
-// at the k_z bins the Ewald pixels need" north_star allows.  A CTA stages a tile of 32 columns by N rows
-// and the twiddle table in shared memory; thread (c, og) accumulates bins s = og, og + 8, ... of column c.
+// at the k_z bins the Ewald pixels need" north_star allows.  A CTA stages a tile of TX columns by N rows
+// and the twiddle table in shared memory; thread (c, og) accumulates bins s = og, og + OG, ... of column c.
 // The phase index k z mod N is stepped in exact integer arithmetic.  O(W N) per column: meant for the
-// short z axes of thin films (N <= 512), not as a general FFT.
-constexpr int DFT_TX = 32, DFT_OG = 8;
+// short z axes of thin films and for lateral sizes that are not powers of two, not as a general FFT.
+// TX columns per tile x OG = 256 / TX bins in flight per column: TX = 32 up to N = 512, TX = 8 beyond (shared memory).
+constexpr int DFT_THREADS = 256;
+__host__ __device__ constexpr int dft_tx(int N) { return N <= 512 ? 32 : 8; }
 
-__global__ void __launch_bounds__(DFT_TX * DFT_OG)
+template <int TX>
+__global__ void __launch_bounds__(DFT_THREADS)
 k_coldft(const ColParams p, int N)
 {
+    constexpr int OG = DFT_THREADS / TX;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2 *sm = reinterpret_cast<float2 *>(smem_raw);       // [N][32]
-    float2 *tw = sm + (size_t)N * DFT_TX;                     // [N]
-    const int tid = threadIdx.x, c = tid % DFT_TX, og = tid / DFT_TX;
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw);       // [N][TX]
+    float2 *tw = sm + (size_t)N * TX;                         // [N]
+    const int tid = threadIdx.x, c = tid % TX, og = tid / TX;
     const int tile = blockIdx.x % p.n_tiles, lo = blockIdx.x / p.n_tiles, hi = blockIdx.y;
-    const float2 *src = p.in + (size_t)hi * p.in_hi + (size_t)lo * p.in_lo + (size_t)tile * DFT_TX + c;
-    for (int z = og; z < N; z += DFT_OG) sm[z * DFT_TX + c] = __ldcs(src + (size_t)z * p.in_row);
-    for (int i = tid; i < N; i += DFT_TX * DFT_OG) tw[i] = p.tw[i];
+    const float2 *src = p.in + (size_t)hi * p.in_hi + (size_t)lo * p.in_lo + (size_t)tile * TX + c;
+    for (int z = og; z < N; z += OG) sm[z * TX + c] = __ldcs(src + (size_t)z * p.in_row);
+    for (int i = tid; i < N; i += DFT_THREADS) tw[i] = p.tw[i];
     __syncthreads();
-    float2 *dst = p.out + (size_t)hi * p.out_hi + (size_t)lo * p.out_lo + (size_t)tile * DFT_TX + c;
-    for (int sl = og; sl < p.win.W; sl += DFT_OG) {
+    float2 *dst = p.out + (size_t)hi * p.out_hi + (size_t)lo * p.out_lo + (size_t)tile * TX + c;
+    for (int sl = og; sl < p.win.W; sl += OG) {
         int k = (p.win.lo + sl) % N;
         if (k < 0) k += N;
-        float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
+        // partial sums over 16 terms are added to the total: the rounding error grows like sqrt(16) + sqrt(N / 16)
+        // ulps instead of sqrt(N) (N up to 2048)
+        float2 tot = make_float2(0.f, 0.f);
         int idx = 0;
-        int z = 0;
-        for (; z + 1 < N; z += 2) {
-            a0 = cfma(sm[z * DFT_TX + c], tw[idx], a0);
-            idx += k; if (idx >= N) idx -= N;
-            a1 = cfma(sm[(z + 1) * DFT_TX + c], tw[idx], a1);
-            idx += k; if (idx >= N) idx -= N;
+        for (int z0 = 0; z0 < N; z0 += 16) {
+            float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
+            const int z1 = min(N, z0 + 16);
+            int z = z0;
+            for (; z + 1 < z1; z += 2) {
+                a0 = cfma(sm[z * TX + c], tw[idx], a0);
+                idx += k; if (idx >= N) idx -= N;
+                a1 = cfma(sm[(z + 1) * TX + c], tw[idx], a1);
+                idx += k; if (idx >= N) idx -= N;
+            }
+            if (z < z1) { a0 = cfma(sm[z * TX + c], tw[idx], a0); idx += k; if (idx >= N) idx -= N; }
+            tot = cadd(tot, cadd(a0, a1));
         }
-        if (z < N) a0 = cfma(sm[z * DFT_TX + c], tw[idx], a0);
-        dst[(size_t)sl * p.out_row] = make_float2(a0.x + a1.x, a0.y + a1.y);
+        dst[(size_t)sl * p.out_row] = tot;
     }
 }
 
@@ -201,6 +212,74 @@ __device__ __forceinline__ void dir_sincos(float x, float *s, float *c)
 #endif
 }
 
+// x pass of SPECTRAL_BASIS for a row length that is not a power of two (DESIGN 3-A14): the definition
+// of Eq. 6 evaluated directly, and only at the window's bins.  One CTA per row; per pack the two real fields of the row are
+// generated into shared memory (kind / material tables of the basis plan), then thread `sl` accumulates bin (lo + sl) mod N.
+// O(W N) per row and pack: a functional path for modest sizes (a 1000 x 1000 film takes a few ms), not a tuned FFT.
+constexpr int XDFT_THREADS = 256;
+
+__device__ __forceinline__ float basis_field(const MorphPtrs &mp, int kind, int m, size_t vox)
+{
+    if (kind == BK_NONE) return 0.f;
+    const float ph = __ldg(mp.phi[m] + vox);
+    if (kind == BK_PHI) return ph;
+    const float w = ph * __ldg(mp.S[m] + vox);
+    if (kind == BK_W) return w;
+    float st, ct, sp, cp;
+    dir_sincos(__ldg(mp.theta[m] + vox), &st, &ct);
+    dir_sincos(__ldg(mp.psi[m] + vox), &sp, &cp);
+    const float dx = cp * st, dy = sp * st, dz = ct;
+    switch (kind) {
+    case BK_XX: return (w * dx) * dx;
+    case BK_YY: return (w * dy) * dy;
+    case BK_XY: return (w * dx) * dy;
+    case BK_XZ: return (w * dx) * dz;
+    default: return (w * dy) * dz;        // BK_YZ
+    }
+}
+
+__global__ void __launch_bounds__(XDFT_THREADS)
+k_xdft(const __grid_constant__ MorphPtrs mp, const int *__restrict__ kind, const int *__restrict__ mat_of, int mat_base, int n_pack,
+       float2 *__restrict__ out, int rows_total, size_t fstride, Window wx, int pitch, const float2 *__restrict__ tw_g, int N)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *f = reinterpret_cast<float2 *>(smem_raw);        // [N] the pack's row
+    float2 *tw = f + N;                                       // [N] exp(-2 pi i t / N)
+    const int tid = threadIdx.x, row = blockIdx.x;
+    if (row >= rows_total) return;
+    for (int i = tid; i < N; i += XDFT_THREADS) tw[i] = tw_g[i];
+    const size_t vox0 = (size_t)row * N;
+    for (int pk = 0; pk < n_pack; ++pk) {
+        __syncthreads();                                     // the previous pack's sums are done with f (and tw is loaded)
+        const int ka = kind[2 * pk], kb = kind[2 * pk + 1], ma = mat_of[2 * pk] - mat_base, mb = mat_of[2 * pk + 1] - mat_base;
+        for (int x = tid; x < N; x += XDFT_THREADS) f[x] = make_float2(basis_field(mp, ka, ma, vox0 + x), basis_field(mp, kb, mb, vox0 + x));
+        __syncthreads();
+        float2 *o = out + (size_t)pk * fstride + (size_t)row * pitch;
+        for (int sl = tid; sl < pitch; sl += XDFT_THREADS) {
+            float2 tot = make_float2(0.f, 0.f);
+            if (sl < wx.W) {
+                int k = (wx.lo + sl) % N;
+                if (k < 0) k += N;
+                int idx = 0;
+                for (int x0 = 0; x0 < N; x0 += 16) {         // partial sums over 16 terms, see k_coldft
+                    float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
+                    const int x1 = min(N, x0 + 16);
+                    int x = x0;
+                    for (; x + 1 < x1; x += 2) {
+                        a0 = cfma(f[x], tw[idx], a0);
+                        idx += k; if (idx >= N) idx -= N;
+                        a1 = cfma(f[x + 1], tw[idx], a1);
+                        idx += k; if (idx >= N) idx -= N;
+                    }
+                    if (x < x1) { a0 = cfma(f[x], tw[idx], a0); idx += k; if (idx >= N) idx -= N; }
+                    tot = cadd(tot, cadd(a0, a1));
+                }
+            }
+            o[sl] = tot;                                     // slots [W, pitch) are the row's zero padding
+        }
+    }
+}
+
 constexpr int XB2_PB = 4;       // packs buffered per row between flushes
 static_assert(XB2_PB >= 4, "an aligned material emits up to 4 packs between flush checks");
 // CTAs per SM the register allocation aims at: 3 (80 registers, a few spilled values) measured 9-12 % faster
@@ -218,7 +297,7 @@ template <int LOGN> struct XB2Cfg {
 
 template <int LOGN>
 __global__ void __launch_bounds__(XB2Cfg<LOGN>::THREADS, XB2_MINB)
-k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, Window wx, int pitch,
+k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, size_t fstride, Window wx, int pitch,
           const float2 *__restrict__ tw)
 {
     using Cfg = XB2Cfg<LOGN>;
@@ -232,7 +311,6 @@ k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
     const int rowc = row_ok ? row : rows_total - 1;
     float2 *Lrow = reinterpret_cast<float2 *>(smem_raw) + (size_t)g * (XB2_PB * N);
     const size_t vox0 = (size_t)rowc * N + li;
-    const size_t fstride = (size_t)rows_total * pitch;
     float2 *orow = out + (size_t)rowc * pitch;
 
     float carry[R0];
@@ -377,11 +455,11 @@ constexpr int XB3_PB = 4;
 #define CYRSOXS_XB3_CTA 128
 #endif
 
-template <int LOGN> struct XB3Cfg {
+template <int LOGN, int CTA> struct XB3CfgT {
     static constexpr int N = 1 << LOGN;
     using F = Fft2<LOGN>;
     static constexpr int T = F::T;
-    static constexpr int ROWS = T >= CYRSOXS_XB3_CTA ? 1 : CYRSOXS_XB3_CTA / T;
+    static constexpr int ROWS = T >= CTA ? 1 : CTA / T;
     static constexpr int THREADS = ROWS * T;
 #ifdef CYRSOXS_XB3_MINB
     static constexpr int MINB = CYRSOXS_XB3_MINB;
@@ -392,24 +470,25 @@ template <int LOGN> struct XB3Cfg {
     static constexpr int RSTRIDE = XB3_PB * LSTRIDE + (N == 64 ? 8 : 0);    // stage / two rows of a half-warp on distinct banks
     static constexpr size_t SMEM = sizeof(float2) * (size_t)ROWS * RSTRIDE;
 };
+template <int LOGN> using XB3Cfg = XB3CfgT<LOGN, CYRSOXS_XB3_CTA>;
 
-template <int LOGN>
-__global__ void __launch_bounds__(XB3Cfg<LOGN>::THREADS, XB3Cfg<LOGN>::MINB)
-k_xbasis3(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, size_t fstride, Window wx, int pitch,
-          const float2 *__restrict__ tws, int rows_ahead)
+// The work of one CTA of the x pass: rows [row_first, row_first + ROWS) of a block of rows_total rows whose first voxel is
+// vox_off (into every morphology array); pack p of row r goes to out[p fstride + r pitch + slot].
+template <int LOGN, int CTA>
+__device__ __forceinline__ void xbasis3_rows(const MorphPtrs &mp, size_t vox_off, float2 *__restrict__ out, int row_first, int rows_total,
+                                             size_t fstride, const Window &wx, int pitch, const float2 *__restrict__ tws, int rows_ahead,
+                                             unsigned char *smem_raw, int tid)
 {
-    using Cfg = XB3Cfg<LOGN>;
+    using Cfg = XB3CfgT<LOGN, CTA>;
     using F = typename Cfg::F;
     using Map = PadMap;
     constexpr int N = Cfg::N, T = Cfg::T, NST = F::NST, THREADS = Cfg::THREADS, LS = Cfg::LSTRIDE;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int tid = threadIdx.x;
     const int g = tid / T, li = tid % T;
-    const int row = blockIdx.x * Cfg::ROWS + g;
+    const int row = row_first + g;
     const bool row_ok = row < rows_total;
     const int rowc = row_ok ? row : rows_total - 1;
     float2 *Lrow = reinterpret_cast<float2 *>(smem_raw) + (size_t)g * Cfg::RSTRIDE;
-    const size_t vox0 = (size_t)rowc * N + li;
+    const size_t vox0 = vox_off + (size_t)rowc * N + li;
     float2 *orow = out + (size_t)rowc * pitch;
 
     float carry[8];
@@ -458,7 +537,7 @@ k_xbasis3(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
     };
     // one 128-byte line per lane: the T threads of a row cover its N floats with N / 32 prefetches per array
     auto prefetch_row_of = [&](const float *a, int r) {
-        if (li < N / 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(a + (size_t)r * N + li * 32));
+        if (li < N / 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(a + vox_off + (size_t)r * N + li * 32));
     };
     auto prefetch_row = [&](const float *a) { prefetch_row_of(a, rowc); };
     // the first material of the rows a later CTA will start with (rows_ahead ~ the rows in flight on the whole GPU):
@@ -525,6 +604,15 @@ k_xbasis3(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int ro
         emit([&](int s) { return carry[s]; }, [](int) { return 0.f; });
     }
     flush();
+}
+
+template <int LOGN>
+__global__ void __launch_bounds__(XB3Cfg<LOGN>::THREADS, XB3Cfg<LOGN>::MINB)
+k_xbasis3(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, size_t fstride, Window wx, int pitch,
+          const float2 *__restrict__ tws, int rows_ahead)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    xbasis3_rows<LOGN, CYRSOXS_XB3_CTA>(mp, 0, out, blockIdx.x * XB3Cfg<LOGN>::ROWS, rows_total, fstride, wx, pitch, tws, rows_ahead, smem_raw, threadIdx.x);
 }
 
 } // namespace cyr

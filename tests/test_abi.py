@@ -35,8 +35,9 @@ def test_no_torch_types_in_signatures():
 
 def test_create_rejects_bad_arguments_without_a_device(lib):
     h = C.c_void_p()
-    for args in [(0, 8, 8, 1, 1.0), (12, 8, 8, 1, 1.0), (8, 12, 8, 1, 1.0), (8, 8, 513, 1, 1.0), (8, 8, 4096, 1, 1.0), (8, 8, 8, 0, 1.0), (8, 8, 8, 33, 1.0),
-                 (8, 8, 8, 1, 0.0), (8, 8, 8, 1, -1.0), (8192, 8, 8, 1, 1.0), (2, 8, 8, 1, 1.0)]:
+    # sizes: 4 <= Nx <= 2048, 2 <= Ny <= 2048, 1 <= Nz <= 2048, any length in between (DESIGN 3-A14)
+    for args in [(0, 8, 8, 1, 1.0), (3, 8, 8, 1, 1.0), (8, 1, 8, 1, 1.0), (8, 8, 0, 1, 1.0), (8, 2049, 8, 1, 1.0), (8, 8, 4096, 1, 1.0), (8, 8, 8, 0, 1.0),
+                 (8, 8, 8, 33, 1.0), (8, 8, 8, 1, 0.0), (8, 8, 8, 1, -1.0), (8192, 8, 8, 1, 1.0), (2, 8, 8, 1, 1.0)]:
         st = lib.cyrsoxs_create(*args, C.byref(h))
         assert st == binding.ERR_INVALID_ARG and not h.value, args
     assert lib.cyrsoxs_create(8, 8, 8, 1, 1.0, None) == binding.ERR_INVALID_ARG

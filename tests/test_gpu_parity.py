@@ -33,6 +33,40 @@ def test_tiny_random(shape, mode, alg):
     compare(out, cnt, ref, rcnt, f"tiny{shape}")
 
 
+@pytest.mark.parametrize("mode", [W.EWALD_NEAREST, W.EWALD_TRILINEAR])
+@pytest.mark.parametrize("shape", [(96, 80, 12), (45, 27, 5), (12, 10, 3), (100, 64, 8), (64, 100, 1), (33, 2, 2), (640, 24, 3), (24, 600, 2)])
+def test_lateral_sizes_that_are_not_powers_of_two(shape, mode):
+    """SURVEY 8(f) NEXT-4 / DESIGN 3-A14: Nx, Ny of any length (pruned direct DFT along such an axis), AUTO algorithm
+    (SPECTRAL_BASIS), both Ewald modes, odd and even sizes, one axis or both, rho = Nx / Ny not a power of two."""
+    nx, ny, nz = shape
+    w = W.tiny(seed=300 + nx + nz, nx=nx, ny=ny, nz=nz, n_mat=3, n_energy=2, voxel_nm=2.0, ewald=mode)
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, ctx = _gpu(w, 0)
+    assert ctx.stats()["algorithm"] == 2
+    compare(out, cnt, ref, rcnt, f"nonpow2{shape}")
+
+
+def test_film_1000x600_not_a_power_of_two():
+    """A 1000 x 600 x 1 film (the reduced cfg4 recipe cannot be cropped, so the random-everything generator): every
+    row and column goes through the direct-DFT passes at a size where their summation order matters."""
+    w = W.tiny(seed=41, nx=1000, ny=600, nz=1, n_mat=3, n_energy=2, voxel_nm=2.0, ewald=W.EWALD_NEAREST, angles=(0.0, 45.0, 135.0))
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, _ = _gpu(w, 0)
+    print("film 1000x600", compare(out, cnt, ref, rcnt, "film1000x600"))
+
+
+def test_per_energy_refuses_nx_that_is_not_a_power_of_two():
+    from paper_2209_13121_b200 import binding
+    w = W.tiny(seed=5, nx=12, ny=8, nz=2, n_mat=2, n_energy=1)
+    with pytest.raises(binding.CyrsoxsError) as ei:
+        binding.simulate(w, algorithm=binding.ALG_PER_ENERGY)
+    assert ei.value.status == binding.ERR_NOT_IMPLEMENTED
+    w2 = W.tiny(seed=5, nx=16, ny=12, nz=6, n_mat=2, n_energy=1)           # Ny, Nz of any length are fine for PER_ENERGY
+    ref, rcnt = oracle_run(w2, linear=True)
+    out, cnt, _ = _gpu(w2, binding.ALG_PER_ENERGY)
+    compare(out, cnt, ref, rcnt, "per-energy 16x12x6")
+
+
 @pytest.mark.parametrize("alg", ALGS)
 def test_stage_images_match_oracle_linear_images(alg):
     w = W.tiny(seed=3, nx=32, ny=32, nz=16, n_mat=3, n_energy=2, voxel_nm=1.0, ewald=W.EWALD_TRILINEAR)
@@ -88,30 +122,33 @@ def test_cfg4_reduced(alg):
     print("cfg4/256", compare(out, cnt, ref, rcnt, "cfg4/256"))
 
 
-def _full_size_sampled(w, energy_idx, label):
+def _full_size_sampled(w, energy_idx, label, chunk=1):
     """Full-size config through the launch configuration bench.py uses (AUTO algorithm, all
     energies in one run); the oracle (linear mode) recomputes the sampled energies one by one."""
     out, cnt, ctx = _gpu(w, 0)
     assert np.isfinite(out).all()
     st = ctx.stats()
-    for e in energy_idx:
-        w1 = w.restrict_energies([e])
-        ref, rcnt = oracle_run(w1, linear=True)
-        r = compare(out[e:e + 1], cnt[e:e + 1], ref, rcnt, f"{label} e={e}")
-        print(label, "energy", e, r, "algorithm", st["algorithm"], "batch", st["energy_batch"])
+    energy_idx = list(energy_idx)
+    for i in range(0, len(energy_idx), chunk):
+        idx = energy_idx[i:i + chunk]
+        ref, rcnt = oracle_run(w.restrict_energies(idx), linear=True)
+        r = compare(out[idx], cnt[idx], ref, rcnt, f"{label} e={idx}")
+        print(label, "energies", idx, {k: float(np.max(v)) for k, v in r.items()}, "algorithm", st["algorithm"], "batch", st["energy_batch"])
 
 
-def test_cfg3_full_size_sampled_energies():
-    """BASELINE configs[2] at full size (512x512x256, 50 energies, trilinear): first, middle and
-    last energy (largest k: the one that sizes the spectral windows) against the oracle."""
+def test_cfg3_full_size_11_of_50_energies():
+    """BASELINE configs[2] at full size (512x512x256, 50 energies, trilinear): 11 energies spread over the grid,
+    both ends included (the last has the largest k: the one that sizes the spectral windows), against the oracle --
+    11 different Ewald geometries (node and validity decisions depend on k)."""
     w = W.cfg3()
-    _full_size_sampled(w, [0, 24, 49], "cfg3")
+    _full_size_sampled(w, [0, 5, 10, 15, 20, 24, 30, 35, 40, 45, 49], "cfg3")
 
 
-def test_cfg4_full_size_sampled_energies():
-    """BASELINE configs[3] at full size (2048x2048x1, 4 materials, 100 energies x 36 angles)."""
+def test_cfg4_full_size_all_100_energies():
+    """BASELINE configs[3] at full size (2048x2048x1, 4 materials, 100 energies x 36 angles): every energy against
+    the linear-mode oracle (2-D: cheap), i.e. 100 different Ewald disks cutting the detector."""
     w = W.cfg4()
-    _full_size_sampled(w, [0, 63, 64, 99], "cfg4")      # 63/64 straddle the energy-batch boundary
+    _full_size_sampled(w, range(w.n_energy), "cfg4", chunk=10)
 
 
 def _host_ram_gb():
@@ -128,16 +165,16 @@ def test_cfg5_quarter_depth_sampled_energies():
     """BASELINE configs[4] at full lateral size and a quarter of the depth (1024x1024x128, 1.3e8
     voxels; same generator, same energies, trilinear).  The full-depth run is the next test."""
     w = W.cfg5(nz=128)
-    _full_size_sampled(w, [0, 19], "cfg5/nz128")
+    _full_size_sampled(w, [0, 10, 19], "cfg5/nz128")
 
 
 @pytest.mark.skipif(_host_ram_gb() < 100.0 or os.environ.get("CYRSOXS_SKIP_FULL_CFG5") == "1",
                     reason="full CFG5 needs ~90 GB of host RAM for the generator and the oracle (about 80 s on the B200 box)")
-def test_cfg5_full_size_sampled_energy():
-    """BASELINE configs[4] at full size (1024x1024x512 = 5.4e8 voxels, 17 GB of morphology):
-    64-bit indexing, memory footprint, the largest windows."""
+def test_cfg5_full_size_first_and_last_energy():
+    """BASELINE configs[4] at full size (1024x1024x512 = 5.4e8 voxels, 17 GB of morphology): 64-bit indexing, memory
+    footprint, the largest windows (last energy) and the low-k end (first energy)."""
     w = W.cfg5()
-    _full_size_sampled(w, [19], "cfg5")
+    _full_size_sampled(w, [0, 19], "cfg5")
 
 
 @pytest.mark.parametrize("alg", ALGS)
