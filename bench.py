@@ -367,6 +367,39 @@ def roofline_of(name, res, peak, peak_src):
                                          "(energy-independent spectra, pruned windows), so frac > 1 is possible"}}
 
 
+def cufft_comparison(w, dev, stage_ms):
+    """cuFFT (through torch.fft.fftn) on the same transforms, as an outside yardstick for the hand-written passes
+    (north_star: "cuFFT may be timed only as a comparison"; it is not on the product path).  One unpruned complex64 3-D
+    transform of the workload's size per basis pack; no field generation, no morphology read, no pruning -- so it is the
+    library's time for the FFT part alone, next to the build's fields + x + z + y passes."""
+    import torch
+    n_fields = sum(7 if m[1] is not None else 1 for m in w.materials)
+    n_pack = (n_fields + 1) // 2
+    try:
+        x = torch.empty((w.Nz, w.Ny, w.Nx), dtype=torch.complex64, device=dev)
+        torch.view_as_real(x).normal_()
+        dims = (-3, -2, -1) if w.Nz > 1 else (-2, -1)
+        for _ in range(2):
+            y = torch.fft.fftn(x, dim=dims)
+        torch.cuda.synchronize(dev)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 3
+        a.record()
+        for _ in range(reps):
+            y = torch.fft.fftn(x, dim=dims)
+        b.record()
+        torch.cuda.synchronize(dev)
+        per = a.elapsed_time(b) / reps
+        del x, y
+        torch.cuda.empty_cache()
+        ours = stage_ms["xpass"] + stage_ms["zpass"] + stage_ms["ypass"]
+        return {"library": "cuFFT via torch.fft.fftn, complex64, unpruned, out of place", "ms_per_transform": per, "n_transforms": n_pack,
+                "ms_total": per * n_pack, "ours_fields_plus_fft_ms": ours, "ours_over_cufft": ours / (per * n_pack),
+                "note": "comparison only; cuFFT is not linked into libcyrsoxs.so"}
+    except Exception as ex:                                  # out of memory on a small device, or no cuFFT
+        return {"unavailable": str(ex)[:200]}
+
+
 def pick_default_workload(dev) -> str:
     """BASELINE.json names no config for the metric: the headline is the largest single-GPU one, configs[4]
     (1024 x 1024 x 512; 17 GB of morphology, 11 GB of workspace, 17 GB pinned for e2e).  A smaller device or
@@ -428,6 +461,8 @@ def run_ours(args, rank, world, local_rank):
         "clocks": res["clocks"],
         "roofline": roofline_of(name, res, peak, peak_src),
     }
+    if world == 1:
+        line["cufft_comparison"] = cufft_comparison(w, dev, res["stage_ms"])
     if world == 1 and not args.no_cpu_baseline:
         v, desc, dt, cores = oracle_sample(w, budget_s=20.0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
@@ -444,7 +479,7 @@ def run_ours(args, rank, world, local_rank):
             per[other] = {"workload": workload_label(wo, other), "ms_per_step": r["ms_per_step"],
                           "patterns_per_s": wo.n_energy * wo.n_angles / (r["ms_per_step"] * 1e-3),
                           "dominant_kernel": rf["kernel"], "frac": rf["frac"], "traffic": rf["traffic"],
-                          "stage_ms_per_step": rf["stage_ms_per_step"],
+                          "stage_ms_per_step": rf["stage_ms_per_step"], "cufft_comparison": cufft_comparison(wo, dev, r["stage_ms"]),
                           "whole_step_frac": rf["whole_step"]["frac"], "whole_step_vs_M0_frac": rf["whole_step_vs_M0"]["frac"]}
             del r, wo
         line["per_config"] = per

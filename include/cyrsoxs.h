@@ -53,7 +53,9 @@ typedef enum {
  *   PER_ENERGY      the paper's order with p linear in e (north_star): per energy the five
  *                   distinct entries of the susceptibility tensor chi (xx, xy, xz, yy, yz; p for
  *                   e = x is its first column, for e = y its second) are formed per voxel,
- *                   transformed, and projected.
+ *                   transformed, and projected.  Kept as the reference organisation (closest to
+ *                   Algorithm 1) and for runs with one energy and many aligned materials; its x
+ *                   pass uses the first-generation FFT core and is not the tuned path.
  *   SPECTRAL_BASIS  p is also linear in the optical constants: the energy-independent real
  *                   fields phi, phi S, phi S d_i d_j are transformed once per run and every
  *                   energy only combines their spectra on its Ewald shell (DESIGN 7.0).
@@ -93,8 +95,10 @@ typedef struct {
  * evaluated at the bins the Ewald step can reach (a pruned direct DFT, O(N W) per line: a functional
  * path for thin films and odd lateral sizes, not a tuned FFT).  Nx that is not a power of two needs
  * CYRSOXS_ALG_SPECTRAL_BASIS (AUTO picks it; PER_ENERGY returns NOT_IMPLEMENTED at run).
- * 1 <= n_mat <= 32, voxel_nm > 0 (else INVALID_ARG).  Uses the current CUDA device.  *out is NULL on failure. */
-cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm, cyrsoxs_ctx **out);
+ * 1 <= n_mat <= 32, voxel_nm > 0 (else INVALID_ARG); voxel_nm is a double because the detector grid dq = 2 pi / (N voxel_nm)
+ * and with it every validity decision is formed in double (DESIGN 3-A11).  Uses the current CUDA device.  *out is NULL on
+ * failure. */
+cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, double voxel_nm, cyrsoxs_ctx **out);
 
 /* Morphology (memory model P:199-203): for each material m four DEVICE arrays of
  * Nx*Ny*Nz float32: volume fraction phi (the paper's v_frac), alignment S, and the director's

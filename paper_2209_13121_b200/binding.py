@@ -55,7 +55,7 @@ def load() -> C.CDLL:
                            "(the CUDA library is the only implementation; there is no CPU fallback)")
     lib = C.CDLL(str(LIB_PATH))
     vp, fpp = C.c_void_p, C.POINTER(C.c_void_p)
-    lib.cyrsoxs_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.POINTER(vp)]
+    lib.cyrsoxs_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(vp)]
     lib.cyrsoxs_set_morphology.argtypes = [vp, fpp, fpp, fpp, fpp]
     lib.cyrsoxs_set_morphology_host.argtypes = [vp, fpp, fpp, fpp, fpp, vp]
     lib.cyrsoxs_set_morphology_aos.argtypes = [vp, vp, vp]

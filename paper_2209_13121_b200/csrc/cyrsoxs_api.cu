@@ -38,7 +38,7 @@ struct DevBuf {
 
 struct cyrsoxs_ctx {
     int Nx = 0, Ny = 0, Nz = 0, n_mat = 0, device = 0, n_sm = 148;
-    float voxel = 0.f;
+    double voxel = 0.0;
     double dqx = 0, dqy = 0, dqz = 0;
     // morphology
     MorphPtrs mp{};
@@ -790,22 +790,22 @@ const char *cyrsoxs_version(void) { return "cyrsoxs-b200 0.1 (sm_100a)"; }
 
 const char *cyrsoxs_last_error(const cyrsoxs_ctx *ctx) { return ctx ? ctx->err.c_str() : kCreateFailed; }
 
-cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, float voxel_nm, cyrsoxs_ctx **out)
+cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, double voxel_nm, cyrsoxs_ctx **out)
 {
     if (!out) return CYRSOXS_ERR_INVALID_ARG;
     *out = nullptr;
     const int maxn = 1 << kMaxLog2;
     static_assert(kMaxAny <= (1 << kMaxLog2), "direct-DFT passes cover every accepted length");
     if (Nx < 4 || Ny < 2 || Nz < 1 || Nx > maxn || Ny > maxn || Nz > maxn) return CYRSOXS_ERR_INVALID_ARG;      // DESIGN 3-A14
-    if (n_mat < 1 || n_mat > MAX_MAT || !(voxel_nm > 0.f) || !isfinite(voxel_nm)) return CYRSOXS_ERR_INVALID_ARG;
+    if (n_mat < 1 || n_mat > MAX_MAT || !(voxel_nm > 0.0) || !isfinite(voxel_nm)) return CYRSOXS_ERR_INVALID_ARG;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CYRSOXS_ERR_CUDA; }
     cyrsoxs_ctx *c = new (std::nothrow) cyrsoxs_ctx();
     if (!c) return CYRSOXS_ERR_OOM;
     c->Nx = Nx; c->Ny = Ny; c->Nz = Nz; c->n_mat = n_mat; c->voxel = voxel_nm; c->device = dev;
-    c->dqx = (2.0 * kPi) / ((double)Nx * (double)voxel_nm);
-    c->dqy = (2.0 * kPi) / ((double)Ny * (double)voxel_nm);
-    c->dqz = (2.0 * kPi) / ((double)Nz * (double)voxel_nm);
+    c->dqx = (2.0 * kPi) / ((double)Nx * voxel_nm);
+    c->dqy = (2.0 * kPi) / ((double)Ny * voxel_nm);
+    c->dqz = (2.0 * kPi) / ((double)Nz * voxel_nm);
     c->mp.n_mat = n_mat;
     if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); c->n_sm = 148; }
     cyrsoxs_status st;

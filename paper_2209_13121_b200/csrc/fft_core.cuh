@@ -9,14 +9,12 @@
 // Stages run in place: every thread reads its butterflies into registers, the block
 // synchronises, then writes.
 //
-// Two shared-memory layouts ("accessors"):
+// Shared-memory layout ("accessor"):
 //   RowAcc  a line is contiguous; re and im in separate float arrays, index i stored at
 //           i + (i >> 5) (one pad word per 32) so that the stride-R writes of the early stages
 //           and the unit-stride reads are both bank-conflict free.  Used by the x pass, where
 //           lanes run along the transform axis.
-//   ColAcc  float2 s[i * TX + column]: lanes run across TX independent columns, so every access
-//           of a (half-)warp is one contiguous 128/256-byte segment.  Used by the strided z and
-//           y passes.
+// (the strided z and y passes keep their lines in registers and in the layouts of fft_reg.cuh)
 #pragma once
 #include <cuda_runtime.h>
 
@@ -153,17 +151,6 @@ template <int N> struct RowAcc {
         int p = line * L::LS + L::pos(i);
         re[p] = v.x; im[p] = v.y;
     }
-};
-
-template <int N, int TX> struct ColAcc {
-    float2 *s;
-    template <int NB> __device__ __forceinline__ static void split(int w, int, int &line, int &j)
-    {
-        line = w % TX; j = w / TX;
-    }
-    __device__ __forceinline__ float2 load(int line, int i) const { return s[i * TX + line]; }
-    __device__ __forceinline__ float2 load_input(int line, int i) const { return s[i * TX + line]; }
-    __device__ __forceinline__ void store(int line, int i, float2 v) const { s[i * TX + line] = v; }
 };
 
 // ---------------------------------------------------------------------------- one stage

@@ -24,10 +24,14 @@ def _gpu(w, alg, images=False):
 
 @pytest.mark.parametrize("alg", ALGS)
 @pytest.mark.parametrize("mode", [W.EWALD_NEAREST, W.EWALD_TRILINEAR])
-@pytest.mark.parametrize("shape", [(8, 8, 4), (32, 16, 8), (16, 64, 2), (64, 32, 1), (4, 4, 16), (16, 512, 2), (8, 4, 512), (1024, 4, 1), (8, 128, 256), (4, 1024, 2), (16, 16, 7), (32, 16, 63), (8, 8, 12), (8, 4, 3), (8, 4, 500)])
+@pytest.mark.parametrize("shape", [(8, 8, 4), (32, 16, 8), (16, 64, 2), (64, 32, 1), (4, 4, 16), (16, 512, 2), (8, 4, 512), (1024, 4, 1), (8, 128, 256), (4, 1024, 2), (16, 16, 7), (32, 16, 63), (8, 8, 12), (8, 4, 3), (8, 4, 500),
+                                   (16, 2, 4), (2048, 4, 2), (4, 2048, 2), (8, 4, 2048), (2048, 2, 8)])
 def test_tiny_random(shape, mode, alg):
+    """Ragged and extreme shapes: Ny = 2, every axis at its maximum of 2048 inside a 3-D model, z axes that are not
+    powers of two; a voxel size that is not representable in float32 (1.3 nm: the ABI takes a double, so the detector
+    grid dq is the oracle's bit for bit)."""
     nx, ny, nz = shape
-    w = W.tiny(seed=100 + nx + nz, nx=nx, ny=ny, nz=nz, n_mat=3, n_energy=3, voxel_nm=2.0, ewald=mode)
+    w = W.tiny(seed=100 + nx + nz, nx=nx, ny=ny, nz=nz, n_mat=3, n_energy=3, voxel_nm=1.3 if nx in (16, 2048) else 2.0, ewald=mode)
     ref, rcnt = oracle_run(w)
     out, cnt, _ = _gpu(w, alg)
     compare(out, cnt, ref, rcnt, f"tiny{shape}")
@@ -346,14 +350,16 @@ def test_degenerate_and_extreme_cases(alg):
     assert (out == 0).all() and (ref == 0).all() and (cnt == rcnt).all()
 
 
+@pytest.mark.parametrize("nx", [32, 40])
 @pytest.mark.parametrize("group", [1, 2, 5])
-def test_streamed_morphology_matches_oracle(group):
+def test_streamed_morphology_matches_oracle(group, nx):
     """cyrsoxs_set_morphology_streamed (NEXT-3, the paper's Algorithm 2/3 idea): materials pass through
     a double-buffered staging area group by group; images within the gates, counts equal, and repeated
-    runs (staging slots reused across runs) give identical images."""
+    runs (staging slots reused across runs) give identical images.  nx = 40: the groups go through the
+    direct-DFT x pass (k_xdft) with their own slice of the basis plan."""
     import torch
     from paper_2209_13121_b200 import binding
-    w = W.tiny(seed=61, nx=32, ny=32, nz=8, n_mat=4, n_energy=3, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR)
+    w = W.tiny(seed=61, nx=nx, ny=32, nz=8, n_mat=4, n_energy=3, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR)
     ref, rcnt = oracle_run(w)
     pinned = [tuple(None if a is None else torch.from_numpy(a).pin_memory() for a in m) for m in w.materials]
     ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
@@ -382,6 +388,41 @@ def test_streamed_morphology_matches_oracle(group):
     ctx.run(out.data_ptr(), s)
     torch.cuda.synchronize()
     compare(out.cpu().numpy(), cnt.cpu().numpy(), ref, rcnt, "resident after streamed")
+    ctx.close()
+
+
+def test_setters_between_runs_on_a_non_blocking_stream_without_sync():
+    """Two runs on a non-blocking side stream with cyrsoxs_set_optical_constants and cyrsoxs_set_angles in between and
+    no synchronisation: the setters only touch host tables, the device copies are refreshed at the next run on its
+    stream (cyrsoxs.h), so the first run's kernels keep the tables they were launched with."""
+    import torch
+    from paper_2209_13121_b200 import binding
+    w = W.tiny(seed=62, nx=64, ny=64, nz=16, n_mat=3, n_energy=4, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR)
+    w2 = W.tiny(seed=63, nx=64, ny=64, nz=16, n_mat=3, n_energy=4, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR, angles=(10.0, 25.0, 160.0))
+    w2.materials = w.materials                               # same morphology, other constants and angles
+    ref1, rcnt1 = oracle_run(w, linear=True)
+    ref2, rcnt2 = oracle_run(w2, linear=True)
+    side = torch.cuda.Stream()                               # non-blocking: not ordered against the legacy stream
+    mats = [tuple(None if a is None else torch.from_numpy(a).cuda() for a in m) for m in w.materials]
+    out1 = torch.empty((4, 64, 64), dtype=torch.float32, device="cuda")
+    out2 = torch.empty_like(out1)
+    cnt1 = torch.zeros((4, 64, 64), dtype=torch.int32, device="cuda")
+    cnt2 = torch.zeros_like(cnt1)
+    torch.cuda.synchronize()
+    ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    ctx.set_morphology(mats)
+    for rep in range(3):
+        ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+        ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald)
+        ctx.set_counts_output(cnt1.data_ptr())
+        ctx.run(out1.data_ptr(), side.cuda_stream)
+        ctx.set_optical_constants(w2.energies, w2.delta_par, w2.beta_par, w2.delta_perp, w2.beta_perp)     # no sync
+        ctx.set_angles(*w2.angles)
+        ctx.set_counts_output(cnt2.data_ptr())
+        ctx.run(out2.data_ptr(), side.cuda_stream)
+    side.synchronize()
+    compare(out1.cpu().numpy(), cnt1.cpu().numpy(), ref1, rcnt1, "first of two back-to-back runs")
+    compare(out2.cpu().numpy(), cnt2.cpu().numpy(), ref2, rcnt2, "second of two back-to-back runs")
     ctx.close()
 
 
