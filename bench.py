@@ -232,7 +232,8 @@ def measure(name, args, rank, world, dev, steps, warmup, with_e2e, with_clocks, 
     import torch
     import torch.distributed as dist
     from paper_2209_13121_b200 import binding
-    w = make_workload(name, rank, world)
+    strong = getattr(args, "scaling", "weak") == "strong" and world > 1
+    w = make_workload(name, 0, 1) if strong else make_workload(name, rank, world)
     local_rank = dev.index
     mats = [tuple(None if a is None else torch.from_numpy(a).to(dev) for a in m) for m in w.materials]
     ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
@@ -256,11 +257,25 @@ def measure(name, args, rank, world, dev, steps, warmup, with_e2e, with_clocks, 
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    if strong:
+        # strong scaling (DESIGN 11): the SAME workload on all ranks; rank r transforms material group r % n_parts,
+        # the pruned spectra are exchanged once per run (NCCL broadcasts on the run's stream), then every rank does
+        # its slice of the energies
+        from paper_2209_13121_b200 import sharding
+        n_parts = min(world, w.n_mat)
+        a_e, b_e = sharding.energy_slices(w.n_energy, world)[rank]
+        ctx.set_spectra_shard(rank % n_parts, n_parts)
+        ctx.set_energy_range(a_e, max(b_e - a_e, 1))
+        out = torch.empty((max(b_e - a_e, 1), w.Ny, w.Nx), dtype=torch.float32, device=dev)
+
     def one_step():
         flush.fill_(1)                                  # L2 flush between timed iterations (outside the events)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
-        ctx.run(out.data_ptr(), sptr)
+        if strong:
+            sharding.run_strong(ctx, w, out, sptr)
+        else:
+            ctx.run(out.data_ptr(), sptr)
         b.record(stream)
         return a, b
 
@@ -285,7 +300,8 @@ def measure(name, args, rank, world, dev, steps, warmup, with_e2e, with_clocks, 
     st = ctx.stats()
     res = {"w": w, "ms_per_step": total_ms / steps, "total_ms": total_ms, "launches_per_step": int(st["kernel_launches"]), "st": st,
            "clocks": sampler.summary() if sampler else None}
-    if args.quick:
+    if args.quick or strong:
+        res["strong"] = strong
         return res
 
     # ---- per-stage device times (CUDA events on the run's stream, inside the library) for the roofline
@@ -436,6 +452,18 @@ def run_ours(args, rank, world, local_rank):
         if world > 1:
             dist.destroy_process_group()
         return
+    if res.get("strong"):
+        # total work is fixed: all energies x angles of the workload, whatever the number of GPUs
+        line = {"metric": METRIC, "value": w.n_energy * w.n_angles / (res["ms_per_step"] * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": workload_label(w, name), "l2": "flushed between timed steps (256 MB write)",
+                           "parallelism": f"spectra sharded over min({world}, {w.n_mat}) material groups, one broadcast of the pruned "
+                                          f"spectra per group and run over NCCL, then energies sharded over {world} GPUs"},
+                "gpu_launches": int(res["launches_per_step"] * args.steps), "clocks": res["clocks"]}
+        print(json.dumps(line), flush=True)
+        dist.destroy_process_group()
+        return
     patterns = w.n_energy * w.n_angles * world
     value = patterns / (res["ms_per_step"] * 1e-3)
     e2e = res["e2e"]
@@ -496,6 +524,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="auto", help="cfg1 .. cfg5; auto: cfg5 (BASELINE.json configs[4]), cfg3 if it does not fit")
     ap.add_argument("--alg", default="auto", choices=["auto", "per_energy", "spectral"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank its own energies of an N-times finer grid (default); strong = the same workload, "
+                         "spectra sharded over materials and exchanged, energies sharded (DESIGN 11)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config key (the other BASELINE.json configs)")
     ap.add_argument("--quick", action="store_true", help="device-timed steps only (no e2e, no per-stage pass, no CPU baseline): the command ncu wraps")

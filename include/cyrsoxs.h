@@ -184,6 +184,37 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *ctx, void *cuda_stream, float *out);
 /* Number of angles currently configured (0 before cyrsoxs_set_angles). */
 int cyrsoxs_num_angles(const cyrsoxs_ctx *ctx);
 
+/* ---- Two-phase run and spectra shards (multi-GPU, DESIGN 11) ------------------------------------------------------
+ * With CYRSOXS_ALG_SPECTRAL_BASIS a run is (1) the energy-independent spectra of the basis fields -- almost all of the
+ * device time on large volumes -- and (2) per energy the Ewald gather and the rotate/average step.  Energies shard over
+ * GPUs without communication, but phase 1 would then be repeated by every GPU; it shards over MATERIALS instead:
+ *
+ *   cyrsoxs_set_spectra_shard(ctx, part, n_parts)   the materials are cut into n_parts contiguous groups of about equal
+ *       field count (7 fields per aligned material, 1 per isotropic one; 1 <= n_parts <= n_mat); this context transforms
+ *       group `part` only.  The fields of a group are paired among themselves (an odd count is padded), so the pack layout
+ *       depends on n_parts, not on `part`: every GPU that sets the same n_parts has the same layout.  Needs a resident
+ *       morphology and SPECTRAL_BASIS (else NOT_IMPLEMENTED at run).  (0, 1) restores the unsharded layout.
+ *   cyrsoxs_set_energy_range(ctx, first, count)     phase 2 (and cyrsoxs_run) processes energies [first, first + count)
+ *       of the tables given to cyrsoxs_set_optical_constants; `out` and the counts buffer then hold `count` images.  The
+ *       spectral windows are always sized for ALL energies of the tables, so GPUs with different ranges share one layout.
+ *       count < 0: all energies (default).
+ *   cyrsoxs_run_spectra(ctx, stream)                phase 1 for this context's part, enqueued on `stream`.
+ *   cyrsoxs_get_spectra(ctx, &d_ptr, &pack_bytes, &n_pack)   the context-owned DEVICE buffer of the pruned spectra,
+ *       n_pack consecutive blocks of pack_bytes ([k_z window][k_y window][x pitch] complex64 each); valid until the next
+ *       change of sizes, constants or shard.  cyrsoxs_get_spectra_part(ctx, part, &first_pack, &n_pack) names the blocks
+ *       a part owns.  The caller copies the other parts' blocks in (NCCL broadcast / all_gather, or cudaMemcpyPeer),
+ *       ordered after phase 1 and before phase 2 on the streams it uses.
+ *   cyrsoxs_run_energies(ctx, stream, out)          phase 2 on whatever the spectra buffer holds (NOT_READY unless
+ *       cyrsoxs_run_spectra ran after the last change of morphology, constants or shard).
+ * cyrsoxs_run is phase 1 followed by phase 2; with a shard of more than one part it produces images from this part's
+ * materials only, so sharded callers use the two calls.  PER_ENERGY: phase 1 is empty, phase 2 does everything. */
+cyrsoxs_status cyrsoxs_set_spectra_shard(cyrsoxs_ctx *ctx, int part, int n_parts);
+cyrsoxs_status cyrsoxs_set_energy_range(cyrsoxs_ctx *ctx, int first, int count);
+cyrsoxs_status cyrsoxs_run_spectra(cyrsoxs_ctx *ctx, void *cuda_stream);
+cyrsoxs_status cyrsoxs_get_spectra(cyrsoxs_ctx *ctx, void **d_spectra, unsigned long long *pack_bytes, int *n_pack);
+cyrsoxs_status cyrsoxs_get_spectra_part(cyrsoxs_ctx *ctx, int part, int *first_pack, int *n_pack);
+cyrsoxs_status cyrsoxs_run_energies(cyrsoxs_ctx *ctx, void *cuda_stream, float *out);
+
 /* Counters of the last run (see cyrsoxs_stats).  Synchronises `cuda_stream` of that run if
  * profiling is enabled. */
 cyrsoxs_status cyrsoxs_get_stats(cyrsoxs_ctx *ctx, cyrsoxs_stats *stats);

@@ -22,6 +22,8 @@ EXPORTS = [
     "cyrsoxs_create", "cyrsoxs_set_morphology", "cyrsoxs_set_morphology_host", "cyrsoxs_set_morphology_aos", "cyrsoxs_set_morphology_streamed",
     "cyrsoxs_set_optical_constants", "cyrsoxs_set_angles", "cyrsoxs_set_ewald", "cyrsoxs_set_algorithm",
     "cyrsoxs_set_counts_output", "cyrsoxs_set_profiling", "cyrsoxs_run", "cyrsoxs_num_angles",
+    "cyrsoxs_set_spectra_shard", "cyrsoxs_set_energy_range", "cyrsoxs_run_spectra", "cyrsoxs_get_spectra", "cyrsoxs_get_spectra_part",
+    "cyrsoxs_run_energies",
     "cyrsoxs_get_stats", "cyrsoxs_reduce", "cyrsoxs_debug_fetch_images", "cyrsoxs_last_error", "cyrsoxs_destroy",
     "cyrsoxs_version",
 ]
@@ -67,6 +69,12 @@ def load() -> C.CDLL:
     lib.cyrsoxs_set_counts_output.argtypes = [vp, vp]
     lib.cyrsoxs_set_profiling.argtypes = [vp, C.c_int]
     lib.cyrsoxs_run.argtypes = [vp, vp, vp]
+    lib.cyrsoxs_set_spectra_shard.argtypes = [vp, C.c_int, C.c_int]
+    lib.cyrsoxs_set_energy_range.argtypes = [vp, C.c_int, C.c_int]
+    lib.cyrsoxs_run_spectra.argtypes = [vp, vp]
+    lib.cyrsoxs_get_spectra.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_ulonglong), C.POINTER(C.c_int)]
+    lib.cyrsoxs_get_spectra_part.argtypes = [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    lib.cyrsoxs_run_energies.argtypes = [vp, vp, vp]
     lib.cyrsoxs_num_angles.argtypes = [vp]
     lib.cyrsoxs_get_stats.argtypes = [vp, C.POINTER(Stats)]
     lib.cyrsoxs_debug_fetch_images.argtypes = [vp, C.c_int, vp]
@@ -196,6 +204,31 @@ class Context:
     # -- run -------------------------------------------------------------------------------
     def run(self, out_ptr: int, stream: int = 0):
         self._check(self.lib.cyrsoxs_run(self.h, C.c_void_p(stream), C.c_void_p(out_ptr)))
+
+    # -- two-phase run, spectra shards (multi-GPU; cyrsoxs.h) -------------------------------
+    def set_spectra_shard(self, part: int, n_parts: int):
+        self._check(self.lib.cyrsoxs_set_spectra_shard(self.h, part, n_parts))
+
+    def set_energy_range(self, first: int, count: int):
+        self._check(self.lib.cyrsoxs_set_energy_range(self.h, first, count))
+
+    def run_spectra(self, stream: int = 0):
+        self._check(self.lib.cyrsoxs_run_spectra(self.h, C.c_void_p(stream)))
+
+    def run_energies(self, out_ptr: int, stream: int = 0):
+        self._check(self.lib.cyrsoxs_run_energies(self.h, C.c_void_p(stream), C.c_void_p(out_ptr)))
+
+    def spectra(self):
+        """(device pointer, bytes per pack, n_pack) of the context-owned pruned spectra."""
+        p, nb, n = C.c_void_p(), C.c_ulonglong(), C.c_int()
+        self._check(self.lib.cyrsoxs_get_spectra(self.h, C.byref(p), C.byref(nb), C.byref(n)))
+        return int(p.value), int(nb.value), int(n.value)
+
+    def spectra_part(self, part: int):
+        """(first pack, number of packs) of a part of the spectra shard."""
+        a, n = C.c_int(), C.c_int()
+        self._check(self.lib.cyrsoxs_get_spectra_part(self.h, part, C.byref(a), C.byref(n)))
+        return int(a.value), int(n.value)
 
     def num_angles(self) -> int:
         return int(self.lib.cyrsoxs_num_angles(self.h))

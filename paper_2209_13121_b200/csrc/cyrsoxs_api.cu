@@ -80,6 +80,13 @@ struct cyrsoxs_ctx {
     std::vector<int> basis_kind, basis_mat;     // [2 n_pack]
     DevBuf d_bcoef, d_bkind, d_bmat;
     bool plan_dirty = true;
+    // spectra shard (cyrsoxs_set_spectra_shard): this context transforms the basis fields of one contiguous group of
+    // materials ("part") of n_parts; the other parts' spectra are written into the buffer by the caller (multi-GPU)
+    int shard_part = 0, shard_parts = 1;
+    std::vector<int> part_m0, part_m1, part_pack0, part_npack;
+    int e_first = 0, e_count = -1;                  // energies processed by run / run_energies (-1: all)
+    bool spectra_ready = false;                     // cyrsoxs_run_spectra has run for the current configuration
+    size_t A3_pack_bytes = 0;                       // bytes of one pack's pruned spectrum in A3
     unsigned long long null_pattern = ~0ull;
     // workspace
     DevBuf A1, A2, A3, img, twx, twy, twz, stage_out[2], red;
@@ -620,17 +627,44 @@ bool is_aligned(const cyrsoxs_ctx *c, int m) { return (c->streamed ? c->host_mp.
 cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c, cudaStream_t st)
 {
     c->basis_kind.clear(); c->basis_mat.clear();
+    // parts of a spectra shard: contiguous material ranges of about equal field count (7 per aligned, 1 per isotropic
+    // material), every part at least one material
+    const int P = c->streamed ? 1 : c->shard_parts;
+    c->part_m0.assign(P, 0); c->part_m1.assign(P, 0); c->part_pack0.assign(P, 0); c->part_npack.assign(P, 0);
+    {
+        int total = 0;
+        for (int m = 0; m < c->n_mat; ++m) total += is_aligned(c, m) ? 7 : 1;
+        int m = 0, cum = 0;
+        for (int q = 0; q < P; ++q) {
+            c->part_m0[q] = m;
+            const int must_leave = P - 1 - q;                 // materials the later parts need
+            const long long target = (long long)total * (q + 1);      // cumulative field count the part should end at, times P
+            for (;;) {
+                cum += is_aligned(c, m) ? 7 : 1; ++m;
+                if (m >= c->n_mat - must_leave) break;
+                // take the next material too if that ends closer to the target (the last part takes everything left)
+                const long long next = (long long)(cum + (is_aligned(c, m) ? 7 : 1)) * P - target, now = (long long)cum * P - target;
+                if (q < P - 1 && llabs(next) >= llabs(now)) break;
+            }
+            c->part_m1[q] = m;
+        }
+    }
+    int part = 0;
     for (int m = 0; m < c->n_mat; ++m) {
+        if (P > 1 && m == c->part_m0[part]) c->part_pack0[part] = (int)c->basis_kind.size() / 2;
         if (is_aligned(c, m)) for (int kd = BK_PHI; kd <= BK_YZ; ++kd) { c->basis_kind.push_back(kd); c->basis_mat.push_back(m); }
         else { c->basis_kind.push_back(BK_PHI); c->basis_mat.push_back(m); }
-        // streamed mode: every material group is transformed by its own launch, so its fields are
-        // paired among themselves and an odd count is padded at the group's end
-        const bool group_end = c->streamed && ((m + 1) % c->stream_group == 0);
+        // streamed mode / sharded spectra: every material group is transformed by its own launch (on its own GPU), so its
+        // fields are paired among themselves and an odd count is padded at the group's end
+        const bool group_end = (c->streamed && ((m + 1) % c->stream_group == 0)) || (P > 1 && m + 1 == c->part_m1[part]);
         if (group_end && (c->basis_kind.size() & 1)) { c->basis_kind.push_back(BK_NONE); c->basis_mat.push_back(0); }
+        if (P > 1 && m + 1 == c->part_m1[part]) { c->part_npack[part] = (int)c->basis_kind.size() / 2 - c->part_pack0[part]; ++part; }
     }
     if (c->basis_kind.size() & 1) { c->basis_kind.push_back(BK_NONE); c->basis_mat.push_back(0); }
     const int pack = (int)c->basis_kind.size() / 2;
     c->n_pack = pack;
+    if (P == 1) { c->part_m1[0] = c->n_mat; c->part_npack[0] = pack; }
+    c->spectra_ready = false;
     const int nb = 2 * pack;
     std::vector<float2> coef((size_t)c->nE * nb);
     for (int e = 0; e < c->nE; ++e)
@@ -661,15 +695,29 @@ cyrsoxs_status build_basis_plan(cyrsoxs_ctx *c, cudaStream_t st)
 cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &wx, const Window &wy, const Window &wz, int pitch)
 {
     const size_t rows = (size_t)c->Ny * c->Nz;
-    const int F = c->n_pack;
-    float2 *A1 = (float2 *)c->A1.p, *A2 = (float2 *)c->A2.p, *A3 = (float2 *)c->A3.p;
+    // this context's part of the basis (all of it unless a spectra shard is set): packs [pk0, pk0 + F), materials [m0, m1)
+    const bool sharded = !c->streamed && c->shard_parts > 1;
+    const int pk0 = sharded ? c->part_pack0[c->shard_part] : 0, F = sharded ? c->part_npack[c->shard_part] : c->n_pack;
+    const int m0s = sharded ? c->part_m0[c->shard_part] : 0, m1s = sharded ? c->part_m1[c->shard_part] : c->n_mat;
+    const size_t fstride1 = rows * (size_t)pitch;
+    float2 *A1 = (float2 *)c->A1.p + (size_t)pk0 * fstride1;
+    float2 *A2 = (float2 *)c->A2.p + (c->Nz > 1 ? (size_t)pk0 * wz.W * c->Ny * pitch : 0);
+    float2 *A3 = (float2 *)c->A3.p + (size_t)pk0 * wz.W * wy.W * pitch;
     const double nvox = (double)c->Nx * c->Ny * c->Nz;
     cyrsoxs_status s;
     double n_iso = 0, n_al = 0;
-    for (int m = 0; m < c->n_mat; ++m) (is_aligned(c, m) ? n_al : n_iso) += 1;
+    for (int m = m0s; m < m1s; ++m) (is_aligned(c, m) ? n_al : n_iso) += 1;
     if (!c->streamed) {
         StageTimer t(c, st, CYRSOXS_STAGE_XPASS);
-        if ((s = launch_xbasis(c, st, c->mp, A1, wx, pitch, (int)rows, rows * (size_t)pitch)) != CYRSOXS_OK) return s;
+        MorphPtrs sub = c->mp;
+        if (sharded) {
+            sub = MorphPtrs{};
+            sub.n_mat = m1s - m0s;
+            for (int m = m0s; m < m1s; ++m) {
+                sub.phi[m - m0s] = c->mp.phi[m]; sub.S[m - m0s] = c->mp.S[m]; sub.theta[m - m0s] = c->mp.theta[m]; sub.psi[m - m0s] = c->mp.psi[m];
+            }
+        }
+        if ((s = launch_xbasis(c, st, sub, A1, wx, pitch, (int)rows, fstride1, pk0, m0s, F)) != CYRSOXS_OK) return s;
     } else {
         // Memory-minimising mode (the paper's Algorithm 2/3 idea): material groups are
         // uploaded into a double-buffered staging area on the copy stream while the previous group's
@@ -682,7 +730,7 @@ cyrsoxs_status run_basis_spectra(cyrsoxs_ctx *c, cudaStream_t st, const Window &
             if (!c->ev_stage_ready[i]) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_stage_ready[i], cudaEventDisableTiming));
             if (!c->ev_stage_free[i]) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_stage_free[i], cudaEventDisableTiming));
         }
-        const size_t fstride = rows * (size_t)pitch;
+        const size_t fstride = fstride1;
         int pack0 = 0, g = 0;
         for (int m0 = 0; m0 < c->n_mat; m0 += G, ++g) {
             const int slot = g & 1, m1 = std::min(c->n_mat, m0 + G);
@@ -845,6 +893,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
 
 static void note_null_pattern(cyrsoxs_ctx *c)
 {
+    c->spectra_ready = false;                // called by every morphology setter: the spectra belong to the old morphology
     unsigned long long pat = 0;
     for (int m = 0; m < c->n_mat; ++m) pat |= (unsigned long long)is_aligned(c, m) << m;
     if (c->streamed) pat ^= 0x8000000000000000ull ^ ((unsigned long long)c->stream_group << 40);
@@ -1148,10 +1197,13 @@ cyrsoxs_status cyrsoxs_set_profiling(cyrsoxs_ctx *c, int enabled)
 
 int cyrsoxs_num_angles(const cyrsoxs_ctx *c) { return c && c->have_angles ? c->nA : 0; }
 
-cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
+// phases: 1 = the energy-independent spectra (SPECTRAL_BASIS), 2 = the energies of the range; cyrsoxs_run does both
+enum { PHASE_SPECTRA = 1, PHASE_ENERGIES = 2 };
+
+static cyrsoxs_status run_impl(cyrsoxs_ctx *c, void *cuda_stream, float *out, int phases)
 {
     if (!c) return CYRSOXS_ERR_INVALID_ARG;
-    if (!out) return fail(c, CYRSOXS_ERR_INVALID_ARG, "out is NULL");
+    if ((phases & PHASE_ENERGIES) && !out) return fail(c, CYRSOXS_ERR_INVALID_ARG, "out is NULL");
     if (!c->have_morph || !c->have_optics || !c->have_angles)
         return fail(c, CYRSOXS_ERR_NOT_READY, "run needs morphology, optical constants and angles (missing:%s%s%s)",
                     c->have_morph ? "" : " morphology", c->have_optics ? "" : " optical-constants", c->have_angles ? "" : " angles");
@@ -1162,12 +1214,19 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     if (c->ran && st != c->last_stream) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_run_done, 0));
 
     // where does `out` live?
-    cudaPointerAttributes pa{};
-    cudaError_t pe = cudaPointerGetAttributes(&pa, out);
-    if (pe != cudaSuccess) { cudaGetLastError(); return fail(c, CYRSOXS_ERR_INVALID_ARG, "out: %s", cudaGetErrorString(pe)); }
-    const bool out_on_host = pa.type == cudaMemoryTypeHost;
-    if (pa.type != cudaMemoryTypeHost && pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
-        return fail(c, CYRSOXS_ERR_INVALID_ARG, "out must be device memory or pinned host memory");
+    bool out_on_host = false;
+    if (phases & PHASE_ENERGIES) {
+        cudaPointerAttributes pa{};
+        cudaError_t pe = cudaPointerGetAttributes(&pa, out);
+        if (pe != cudaSuccess) { cudaGetLastError(); return fail(c, CYRSOXS_ERR_INVALID_ARG, "out: %s", cudaGetErrorString(pe)); }
+        out_on_host = pa.type == cudaMemoryTypeHost;
+        if (pa.type != cudaMemoryTypeHost && pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
+            return fail(c, CYRSOXS_ERR_INVALID_ARG, "out must be device memory or pinned host memory");
+    }
+    // the energies this call processes (cyrsoxs_set_energy_range); windows and tables always cover all of them
+    const int e_first = c->e_count < 0 ? 0 : c->e_first, nE_run = c->e_count < 0 ? c->nE : c->e_count;
+    if (e_first < 0 || nE_run < 1 || e_first + nE_run > c->nE)
+        return fail(c, CYRSOXS_ERR_INVALID_ARG, "energy range [%d, %d) is not inside the %d energies set", e_first, e_first + nE_run, c->nE);
 
     cyrsoxs_status s;
     if ((s = upload_tables(c, st)) != CYRSOXS_OK) return s;
@@ -1192,13 +1251,16 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     const size_t npix = (size_t)c->Nx * c->Ny;
     const size_t F1 = spectral ? (size_t)c->n_pack : (size_t)NCHI;
     const size_t a1 = F1 * c->Nz * c->Ny * pitch, a2 = c->Nz > 1 ? F1 * wz.W * c->Ny * pitch : 0, a3 = F1 * wz.W * wy.W * pitch;
+    c->A3_pack_bytes = sizeof(float2) * (size_t)wz.W * wy.W * pitch;
     const size_t per_img = sizeof(float4) * npix + (out_on_host ? 2 * sizeof(float) * npix : 0);
     const size_t per_e = spectral ? per_img : sizeof(float2) * (a1 + a2 + a3) + per_img;
     const size_t stage_bytes = c->streamed ? 2 * (size_t)c->stream_group * 4 * sizeof(float) * (size_t)c->Nx * c->Ny * c->Nz : 0;
     const size_t fixed = (spectral ? sizeof(float2) * (a1 + a2 + a3) : 0) + stage_bytes;
     // The energy batch depends on the free device memory; cudaMemGetInfo is slow, so the batch is
     // re-planned only when what it depends on has changed since the last run.
-    const unsigned long long plan_key = (unsigned long long)c->nE * 8 + (spectral ? 4 : 0) + (out_on_host ? 2 : 0) + 1;
+    if (c->shard_parts > 1 && !spectral)
+        return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "a spectra shard needs CYRSOXS_ALG_SPECTRAL_BASIS (or AUTO) and a resident morphology");
+    const unsigned long long plan_key = (unsigned long long)nE_run * 8 + (spectral ? 4 : 0) + (out_on_host ? 2 : 0) + 1;
     int eb = c->plan_eb;
     if (plan_key != c->plan_key || fixed != c->plan_fixed || per_e != c->plan_per_e || eb < 1) {
         size_t free_b = 0, total_b = 0;
@@ -1209,7 +1271,7 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
         if (fixed + per_e > budget)
             return fail(c, CYRSOXS_ERR_OOM, "workspace of %.1f GB does not fit in %.1f GB of free device memory",
                         (double)(fixed + per_e) / 1e9, (double)budget / 1e9);
-        eb = (int)std::min<size_t>((size_t)c->nE, std::max<size_t>(1, (budget - fixed) / per_e));
+        eb = (int)std::min<size_t>((size_t)nE_run, std::max<size_t>(1, (budget - fixed) / per_e));
         if (!spectral) {
             // ~2 GiB of fields per batch is plenty of parallelism
             const size_t target = (size_t)1 << 31;
@@ -1219,7 +1281,7 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
             eb = (int)std::max<size_t>(1, std::min<size_t>((size_t)eb, std::max<size_t>(1, target / per_img)));
         }
         eb = std::min(eb, 256);
-        if (eb < c->nE && eb >= 8) eb = eb / 8 * 8;               // whole image groups in all but the last batch
+        if (eb < nE_run && eb >= 8) eb = eb / 8 * 8;              // whole image groups in all but the last batch
         c->plan_key = plan_key; c->plan_fixed = fixed; c->plan_per_e = per_e; c->plan_eb = eb;
     }
     c->eg = choose_eg(eb);
@@ -1242,17 +1304,22 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     clear_prof(c);
     memset(&c->stats, 0, sizeof c->stats);
     c->stats.algorithm = alg;
-    c->stats.n_energy = c->nE; c->stats.n_angles = c->nA; c->stats.energy_batch = eb;
+    c->stats.n_energy = nE_run; c->stats.n_angles = c->nA; c->stats.energy_batch = eb;
     c->stats.workspace_bytes = (double)(c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap);
     c->last_stream = st;
 
-    if (spectral && (s = run_basis_spectra(c, st, wx, wy, wz, pitch)) != CYRSOXS_OK) return s;
+    if (phases & PHASE_SPECTRA) {
+        if (spectral && (s = run_basis_spectra(c, st, wx, wy, wz, pitch)) != CYRSOXS_OK) return s;
+        c->spectra_ready = true;
+    } else if (spectral && !c->spectra_ready)
+        return fail(c, CYRSOXS_ERR_NOT_READY, "cyrsoxs_run_energies needs cyrsoxs_run_spectra first (after the last change of morphology, constants or shard)");
 
     int nb = 0;
-    for (int e0 = 0; e0 < c->nE; e0 += eb, ++nb) {
-        const int n = std::min(eb, c->nE - e0);
-        unsigned int *cnt = c->d_counts ? c->d_counts + (size_t)e0 * npix : nullptr;
-        float *dst = out + (size_t)e0 * npix;
+    for (int e0 = e_first; (phases & PHASE_ENERGIES) && e0 < e_first + nE_run; e0 += eb, ++nb) {
+        const int n = std::min(eb, e_first + nE_run - e0);
+        // `out` and the counts buffer hold the energies of the range only
+        unsigned int *cnt = c->d_counts ? c->d_counts + (size_t)(e0 - e_first) * npix : nullptr;
+        float *dst = out + (size_t)(e0 - e_first) * npix;
         const int slot = nb & 1;
         if (out_on_host) {
             // the staging slot is free once the copy issued two batches ago has finished
@@ -1264,7 +1331,7 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
         if (out_on_host) {
             CUDA_TRY(c, cudaEventRecord(c->ev_batch[slot], st));
             CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_batch[slot], 0));
-            CUDA_TRY(c, cudaMemcpyAsync(out + (size_t)e0 * npix, dst, sizeof(float) * npix * n, cudaMemcpyDeviceToHost, c->copy_stream));
+            CUDA_TRY(c, cudaMemcpyAsync(out + (size_t)(e0 - e_first) * npix, dst, sizeof(float) * npix * n, cudaMemcpyDeviceToHost, c->copy_stream));
             CUDA_TRY(c, cudaEventRecord(c->ev_copy[slot], c->copy_stream));
         }
         c->last_batch_e = n;
@@ -1275,6 +1342,51 @@ cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out)
     }
     CUDA_TRY(c, cudaEventRecord(c->ev_run_done, st));
     c->ran = true;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_run(cyrsoxs_ctx *c, void *cuda_stream, float *out) { return run_impl(c, cuda_stream, out, PHASE_SPECTRA | PHASE_ENERGIES); }
+
+cyrsoxs_status cyrsoxs_run_spectra(cyrsoxs_ctx *c, void *cuda_stream) { return run_impl(c, cuda_stream, nullptr, PHASE_SPECTRA); }
+
+cyrsoxs_status cyrsoxs_run_energies(cyrsoxs_ctx *c, void *cuda_stream, float *out) { return run_impl(c, cuda_stream, out, PHASE_ENERGIES); }
+
+cyrsoxs_status cyrsoxs_set_spectra_shard(cyrsoxs_ctx *c, int part, int n_parts)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (n_parts < 1 || n_parts > c->n_mat || part < 0 || part >= n_parts)
+        return fail(c, CYRSOXS_ERR_INVALID_ARG, "spectra shard: 1 <= n_parts <= n_mat (%d) and 0 <= part < n_parts", c->n_mat);
+    c->shard_part = part; c->shard_parts = n_parts;
+    c->plan_dirty = true;
+    c->spectra_ready = false;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_set_energy_range(cyrsoxs_ctx *c, int first, int count)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (count >= 0 && (first < 0 || count < 1)) return fail(c, CYRSOXS_ERR_INVALID_ARG, "energy range: first >= 0 and count >= 1 (or count < 0 for all)");
+    c->e_first = count < 0 ? 0 : first; c->e_count = count < 0 ? -1 : count;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_get_spectra(cyrsoxs_ctx *c, void **d_spectra, unsigned long long *pack_bytes, int *n_pack)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (!c->spectra_ready || !c->A3.p) return fail(c, CYRSOXS_ERR_NOT_READY, "no spectra yet: call cyrsoxs_run_spectra first");
+    if (d_spectra) *d_spectra = c->A3.p;
+    if (pack_bytes) *pack_bytes = (unsigned long long)c->A3_pack_bytes;
+    if (n_pack) *n_pack = c->n_pack;
+    return CYRSOXS_OK;
+}
+
+cyrsoxs_status cyrsoxs_get_spectra_part(cyrsoxs_ctx *c, int part, int *first_pack, int *n_pack)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (!c->spectra_ready) return fail(c, CYRSOXS_ERR_NOT_READY, "no spectra yet: call cyrsoxs_run_spectra first");
+    if (part < 0 || part >= (int)c->part_pack0.size()) return fail(c, CYRSOXS_ERR_INVALID_ARG, "no such part");
+    if (first_pack) *first_pack = c->part_pack0[part];
+    if (n_pack) *n_pack = c->part_npack[part];
     return CYRSOXS_OK;
 }
 

@@ -1,4 +1,13 @@
-"""Energy sharding over ranks (energies are independent,
+"""Sharding over ranks.  Two partitions:
+
+* energies -- no data-path collective, every rank holds the full morphology;
+* the energy-independent spectra of SPECTRAL_BASIS over MATERIALS (`material_parts`, `exchange_spectra`,
+  `simulate_strong`): after reduction R4 almost all device time of a large run is the transform of the basis fields,
+  which energy sharding would repeat on every rank.  Rank r transforms the fields of material group r, the pruned
+  spectra (the Ewald windows: 0.77 GB at CFG3, 3.6 GB at CFG5) are exchanged once per run over NVLink (one broadcast per
+  group), then every rank does its slice of the energies.
+
+Energy sharding over ranks (energies are independent,
 "embarrassingly parallel", one GPU per energy chunk, morphology replicated).
 
 Host-side logic only -- which energies a rank owns and how the per-rank image stacks are
@@ -9,7 +18,7 @@ communication is the optional gather of the finished images (Ny*Nx floats per en
 """
 from __future__ import annotations
 
-from typing import List, Optional, Tuple
+from typing import List, Optional, Sequence, Tuple
 
 
 def energy_slices(n_energy: int, world: int) -> List[Tuple[int, int]]:
@@ -74,3 +83,99 @@ def simulate_sharded(workload, algorithm: int = 0, device: Optional[str] = None,
     if not gather:
         return local
     return gather_images(local, workload.n_energy, 0, group)
+
+
+# ----------------------------------------------------------------------------- spectra shards (strong scaling)
+
+def material_parts(aligned: Sequence[bool], n_parts: int) -> List[Tuple[int, int]]:
+    """Contiguous material ranges [m0, m1), one per part, of about equal basis-field count (7 fields per aligned
+    material, 1 per isotropic one), every part at least one material.  The same rule as the library's
+    (cyrsoxs_set_spectra_shard; `Context.spectra_part` reports the library's pack ranges)."""
+    n_mat = len(aligned)
+    if not 1 <= n_parts <= n_mat:
+        raise ValueError("1 <= n_parts <= number of materials")
+    w = [7 if a else 1 for a in aligned]
+    total = sum(w)
+    out, m, cum = [], 0, 0
+    for q in range(n_parts):
+        m0 = m
+        must_leave = n_parts - 1 - q
+        target = total * (q + 1)                                   # cumulative field count this part should end at, times n_parts
+        while True:
+            cum += w[m]
+            m += 1
+            if m >= n_mat - must_leave:
+                break
+            # take the next material too if that ends closer to the target (the last part takes everything left)
+            if q < n_parts - 1 and abs((cum + w[m]) * n_parts - target) >= abs(cum * n_parts - target):
+                break
+        out.append((m0, m))
+    return out
+
+
+def pack_ranges(aligned: Sequence[bool], n_parts: int) -> List[Tuple[int, int]]:
+    """(first pack, number of packs) of every part: the fields of a part are paired among themselves, an odd count
+    is padded (n_parts = 1: all fields in one sequence)."""
+    out, first = [], 0
+    for m0, m1 in material_parts(aligned, n_parts):
+        fields = sum(7 if a else 1 for a in aligned[m0:m1])
+        n = (fields + 1) // 2
+        out.append((first, n))
+        first += n
+    return out
+
+
+def owner_of_part(part: int, world: int) -> int:
+    """The rank whose transform of `part` is the one that is broadcast (ranks beyond the number of parts repeat a
+    part concurrently and only receive)."""
+    return part % world
+
+
+def exchange_spectra(spectra, ranges: Sequence[Tuple[int, int]], group=None):
+    """spectra: [n_pack, ...] tensor, on every rank the block of its own part filled in.  One broadcast per part
+    from its owner; afterwards every rank holds all blocks.  Returns the bytes this rank received."""
+    import torch.distributed as dist
+    world, rank = dist.get_world_size(group), dist.get_rank(group)
+    received = 0
+    for part, (first, n) in enumerate(ranges):
+        if n == 0:
+            continue
+        block = spectra[first:first + n]
+        src = owner_of_part(part, world)
+        dist.broadcast(block, src=src if group is None else dist.get_global_rank(group, src), group=group)
+        if rank != src:
+            received += block.numel() * block.element_size()
+    return received
+
+
+class _DevicePtr:
+    """CUDA array interface over a raw device pointer (the library owns the memory)."""
+    def __init__(self, ptr: int, nbytes: int):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+
+
+def spectra_tensor(ctx):
+    """The context-owned spectra buffer as a [n_pack, pack_bytes] uint8 CUDA tensor (no copy)."""
+    import torch
+    ptr, pack_bytes, n_pack = ctx.spectra()
+    return torch.as_tensor(_DevicePtr(ptr, pack_bytes * n_pack), device="cuda").view(n_pack, pack_bytes)
+
+
+def run_strong(ctx, workload, out, stream_ptr: int, group=None):
+    """One strong-scaling run on this rank: its part of the spectra, the exchange, its slice of the energies into
+    `out` [n_local][Ny][Nx].  `ctx` has the full morphology, ALL energies of the workload, angles and Ewald mode set,
+    its shard set to (rank % n_parts, n_parts) and its energy range to the rank's slice.  Returns bytes received."""
+    import torch.distributed as dist
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    ctx.run_spectra(stream_ptr)
+    received = 0
+    if world > 1:
+        aligned = [m[1] is not None for m in workload.materials]
+        n_parts = min(world, len(aligned))
+        spec = spectra_tensor(ctx)
+        ranges = [ctx.spectra_part(q) for q in range(n_parts)]
+        assert ranges == pack_ranges(aligned, n_parts), "library and host disagree on the pack layout"
+        received = exchange_spectra(spec, ranges, group)          # on torch's current stream == the run's stream
+    if out is not None and out.shape[0] > 0:
+        ctx.run_energies(out.data_ptr(), stream_ptr)
+    return received

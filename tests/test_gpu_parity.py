@@ -541,3 +541,65 @@ def test_P14_footprint_bound(shape, n_mat, n_energy):
     ctx.run(out.data_ptr(), torch.cuda.current_stream().cuda_stream)
     torch.cuda.synchronize()
     assert ctx.stats()["workspace_bytes"] == ws
+
+
+@pytest.mark.parametrize("n_mat,n_parts", [(2, 2), (4, 2), (4, 3), (3, 3)])
+def test_spectra_shards_and_energy_ranges_match_oracle(n_mat, n_parts):
+    """The strong-scaling path of DESIGN 11 on ONE GPU, its ranks emulated one after the other (nothing waits on anything):
+    context q transforms material group q (cyrsoxs_set_spectra_shard, cyrsoxs_run_spectra), the blocks of the other
+    groups are copied in from their owners' buffers (the broadcast of sharding.exchange_spectra as device copies), then
+    every context runs its own energy range (cyrsoxs_run_energies) -- images and counts against the oracle."""
+    import torch
+    from paper_2209_13121_b200 import binding, sharding
+    w = W.tiny(seed=90 + n_mat, nx=64, ny=32, nz=16, n_mat=n_mat, n_energy=5, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR, isotropic_last=True)
+    ref, rcnt = oracle_run(w, linear=True)
+    aligned = [m[1] is not None for m in w.materials]
+    s = torch.cuda.current_stream().cuda_stream
+    mats = [tuple(None if a is None else torch.from_numpy(a).cuda() for a in m) for m in w.materials]
+    slices = sharding.energy_slices(w.n_energy, n_parts)
+    ctxs, specs = [], []
+    for q in range(n_parts):
+        ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+        ctx.set_morphology(mats)
+        ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)     # ALL energies
+        ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald)
+        ctx.set_spectra_shard(q, n_parts)
+        ctx.set_energy_range(slices[q][0], slices[q][1] - slices[q][0])
+        ctx.run_spectra(s)
+        ranges = [ctx.spectra_part(p) for p in range(n_parts)]
+        assert ranges == sharding.pack_ranges(aligned, n_parts)
+        ctxs.append(ctx); specs.append(sharding.spectra_tensor(ctx))
+    torch.cuda.synchronize()
+    assert all(sp.shape == specs[0].shape for sp in specs)
+    for q in range(n_parts):                                        # "broadcast" part p from its owner p to everybody
+        for p, (first, n) in enumerate(ranges):
+            if p != q:
+                specs[q][first:first + n].copy_(specs[p][first:first + n])
+    for q in range(n_parts):
+        a, b = slices[q]
+        out = torch.empty((b - a, w.Ny, w.Nx), dtype=torch.float32, device="cuda")
+        cnt = torch.zeros((b - a, w.Ny, w.Nx), dtype=torch.int32, device="cuda")
+        ctxs[q].set_counts_output(cnt.data_ptr())
+        ctxs[q].run_energies(out.data_ptr(), s)
+        torch.cuda.synchronize()
+        compare(out.cpu().numpy(), cnt.cpu().numpy(), ref[a:b], rcnt[a:b], f"shard {q}/{n_parts}")
+    # run_energies without spectra is refused; an energy range outside the tables too
+    fresh = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    fresh.set_morphology(mats)
+    fresh.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    fresh.set_angles(*w.angles)
+    out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.CyrsoxsError) as ei:
+        fresh.run_energies(out.data_ptr(), s)
+    assert ei.value.status == binding.ERR_NOT_READY
+    fresh.set_energy_range(3, 4)
+    with pytest.raises(binding.CyrsoxsError) as ei:
+        fresh.run(out.data_ptr(), s)
+    assert ei.value.status == binding.ERR_INVALID_ARG
+    # an energy range through plain cyrsoxs_run
+    fresh.set_energy_range(1, 3)
+    fresh.run(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    compare(out[:3].cpu().numpy(), None, ref[1:4], rcnt[1:4], "energy range 1..3")
+    for c in ctxs + [fresh]:
+        c.close()

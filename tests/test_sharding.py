@@ -91,3 +91,67 @@ def test_gloo_sharded_run_matches_single_process(world, n_energy):
                         w.angles, w.ewald)
     assert full.shape == ref.shape
     assert np.array_equal(full, ref)
+
+
+# ----------------------------------------------------------------------------- spectra shards (strong scaling)
+
+def test_material_parts_cover_balance_and_pack_layout():
+    cases = [([True, True], 2), ([True, True, False], 2), ([True, True, False, False], 3), ([False] * 5, 5),
+             ([True, False, False, False, True], 2), ([False] * 5, 2), ([True] * 4 + [False] * 3, 3), ([True, True, False], 1)]
+    for aligned, n_parts in cases:
+        parts = sharding.material_parts(aligned, n_parts)
+        assert len(parts) == n_parts and parts[0][0] == 0 and parts[-1][1] == len(aligned)
+        assert all(parts[i][1] == parts[i + 1][0] for i in range(n_parts - 1)) and all(b > a for a, b in parts)
+        fields = [sum(7 if x else 1 for x in aligned[a:b]) for a, b in parts]
+        assert max(fields) - min(fields) <= 7, (aligned, parts)           # no part is off by more than one material's worth
+        ranges = sharding.pack_ranges(aligned, n_parts)
+        assert ranges[0][0] == 0 and all(ranges[i][0] + ranges[i][1] == ranges[i + 1][0] for i in range(n_parts - 1))
+        assert [n for _, n in ranges] == [(f + 1) // 2 for f in fields]
+    assert sharding.material_parts([True, True, False], 2) == [(0, 1), (1, 3)]   # 7 | 8 fields, not 14 | 1
+    with pytest.raises(ValueError):
+        sharding.material_parts([True], 2)
+
+
+def _spectra_worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        aligned = [True, False, True, False, False]
+        n_parts = min(world, len(aligned))
+        ranges = sharding.pack_ranges(aligned, n_parts)
+        n_pack = ranges[-1][0] + ranges[-1][1]
+        spec = torch.full((n_pack, 6), -1.0)
+        for part, (first, n) in enumerate(ranges):                   # what this rank "transformed": its own part(s)
+            if part % world == rank:
+                spec[first:first + n] = torch.arange(first, first + n, dtype=torch.float32)[:, None] * 10 + torch.arange(6.0)
+        got = sharding.exchange_spectra(spec, ranges)
+        q.put((rank, spec.numpy(), got))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_gloo_exchange_of_spectra_parts(world):
+    """Every rank ends with every part's block (one broadcast per part from its owner) and counts its received bytes."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_spectra_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=120) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    aligned = [True, False, True, False, False]
+    ranges = sharding.pack_ranges(aligned, min(world, len(aligned)))
+    n_pack = ranges[-1][0] + ranges[-1][1]
+    expect = np.arange(n_pack, dtype=np.float32)[:, None] * 10 + np.arange(6, dtype=np.float32)
+    for rank, spec, got in res:
+        assert np.array_equal(spec, expect), rank
+        own = sum(n for part, (_, n) in enumerate(ranges) if part % world == rank)
+        assert got == (n_pack - own) * 6 * 4
