@@ -16,6 +16,16 @@ namespace cyr {
 
 constexpr int MAX_MAT = 32;
 
+// First statement of every kernel of the path.  The host launches them with programmatic dependent launch allowed
+// (launch_pdl in cyrsoxs_api.cu): the grid may start while the previous kernel of the stream is still draining.
+// griddepcontrol.wait blocks until that kernel has completed and its writes are visible (a no-op for a plain launch);
+// launch_dependents lets the NEXT kernel of the stream be scheduled as soon as all CTAs of this one have started.
+__device__ __forceinline__ void pdl_entry()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 // Bins k in [lo, lo + W) (mod N) of a transformed axis are kept, bin k at slot (k - lo) mod N.
 struct Window {
     int N, lo, W;
@@ -65,6 +75,7 @@ k_xpass_chi(const __grid_constant__ MorphPtrs mp, const float *__restrict__ coef
             float2 *__restrict__ out, int rows_total, Window wx, int pitch,
             const float2 *__restrict__ tw_g)
 {
+    pdl_entry();
     using Cfg = XCfg<LOGN>;
     constexpr int N = Cfg::N;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -287,6 +298,7 @@ template <int EG>
 __global__ void __launch_bounds__(256)
 k_ewald_chi(const EwaldParams p)
 {
+    pdl_entry();
     using M = EwaldMap<EG>;
     const int sub = threadIdx.x % EG, pp = threadIdx.x / EG;
     const int ix = blockIdx.x * M::PW + pp % M::PW;
@@ -336,6 +348,7 @@ template <int EG>
 __global__ void __launch_bounds__(256)
 k_ewald_basis(const EwaldBasisParams q)
 {
+    pdl_entry();
     using M = EwaldMap<EG>;
     const EwaldParams &p = q.g;
     const int sub = threadIdx.x % EG, pp = threadIdx.x / EG;
@@ -406,6 +419,7 @@ template <int EG>
 __global__ void __launch_bounds__(256)
 k_ewald_basis_2d(const EwaldBasisParams q)
 {
+    pdl_entry();
     const EwaldParams &p = q.g;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nb = 2 * q.n_pack, ne = p.n_e;
@@ -534,6 +548,7 @@ template <int EG, int UA, int MINB, int AS>
 __global__ void __launch_bounds__(256, MINB)
 k_rotate_avg(const RotateParams p)
 {
+    pdl_entry();
     using M = RotMap<EG, AS>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n_groups = (p.n_energy + EG - 1) / EG;

@@ -26,6 +26,7 @@ template <int LOGN>
 __global__ void __launch_bounds__(Col2Cfg<LOGN>::THREADS)
 k_col2(const ColParams p)
 {
+    pdl_entry();
     using Cfg = Col2Cfg<LOGN>;
     using F = typename Cfg::F;
     constexpr int N = Cfg::N, TX = Cfg::TX, T = Cfg::T, R0 = F::R0, NST = F::NST;
@@ -87,6 +88,7 @@ template <int LOGN, int PW_>
 __global__ void __launch_bounds__(Col2PCfg<LOGN, PW_>::THREADS)
 k_col2p(const ColParams p)
 {
+    pdl_entry();
     using Cfg = Col2PCfg<LOGN, PW_>;
     using F = typename Cfg::F;
     constexpr int N = Cfg::N, TX = Cfg::TX, PW = Cfg::PW, T = Cfg::T, R0 = F::R0, NST = F::NST;
@@ -152,6 +154,7 @@ template <int TX>
 __global__ void __launch_bounds__(DFT_THREADS)
 k_coldft(const ColParams p, int N)
 {
+    pdl_entry();
     constexpr int OG = DFT_THREADS / TX;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *sm = reinterpret_cast<float2 *>(smem_raw);       // [N][TX]
@@ -242,6 +245,7 @@ __global__ void __launch_bounds__(XDFT_THREADS)
 k_xdft(const __grid_constant__ MorphPtrs mp, const int *__restrict__ kind, const int *__restrict__ mat_of, int mat_base, int n_pack,
        float2 *__restrict__ out, int rows_total, size_t fstride, Window wx, int pitch, const float2 *__restrict__ tw_g, int N)
 {
+    pdl_entry();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *f = reinterpret_cast<float2 *>(smem_raw);        // [N] the pack's row
     float2 *tw = f + N;                                       // [N] exp(-2 pi i t / N)
@@ -300,6 +304,7 @@ __global__ void __launch_bounds__(XB2Cfg<LOGN>::THREADS, XB2_MINB)
 k_xbasis2(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, size_t fstride, Window wx, int pitch,
           const float2 *__restrict__ tw)
 {
+    pdl_entry();
     using Cfg = XB2Cfg<LOGN>;
     using F = typename Cfg::F;
     constexpr int N = Cfg::N, T = Cfg::T, R0 = Cfg::R0, NST = F::NST, THREADS = Cfg::THREADS;
@@ -611,6 +616,7 @@ __global__ void __launch_bounds__(XB3Cfg<LOGN>::THREADS, XB3Cfg<LOGN>::MINB)
 k_xbasis3(const __grid_constant__ MorphPtrs mp, float2 *__restrict__ out, int rows_total, size_t fstride, Window wx, int pitch,
           const float2 *__restrict__ tws, int rows_ahead)
 {
+    pdl_entry();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     xbasis3_rows<LOGN, CYRSOXS_XB3_CTA>(mp, 0, out, blockIdx.x * XB3Cfg<LOGN>::ROWS, rows_total, fstride, wx, pitch, tws, rows_ahead, smem_raw, threadIdx.x);
 }

@@ -603,3 +603,43 @@ def test_spectra_shards_and_energy_ranges_match_oracle(n_mat, n_parts):
     compare(out[:3].cpu().numpy(), None, ref[1:4], rcnt[1:4], "energy range 1..3")
     for c in ctxs + [fresh]:
         c.close()
+
+
+def _random_case(i):
+    """Seeded random small case: sizes (powers of two or not), 1-6 materials with a random aligned / isotropic pattern,
+    1-12 energies, voxel sizes from 0.3 to 8 nm (Ewald disk far inside the detector ... far outside), both Ewald modes,
+    random angle lists."""
+    rng = np.random.default_rng(7000 + i)
+    sizes = [4, 6, 8, 12, 16, 20, 32, 33, 48, 64, 96, 100, 128]
+    nx, ny = int(rng.choice(sizes)), int(rng.choice([2, 3] + sizes))
+    nz = int(rng.choice([1, 1, 2, 3, 4, 5, 8, 16, 17, 32]))
+    n_mat = int(rng.integers(1, 7))
+    n_energy = int(rng.integers(1, 13))
+    voxel = float(rng.choice([0.3, 0.7, 1.0, 1.3, 2.0, 3.7, 8.0]))
+    mode = int(rng.integers(0, 2))
+    start = float(rng.choice([0.0, 0.0, 7.5, -30.0]))
+    step = float(rng.choice([5.0, 15.0, 22.5, 45.0, 90.0]))
+    end = start + step * int(rng.integers(0, 12))
+    w = W.tiny(seed=8000 + i, nx=nx, ny=ny, nz=nz, n_mat=n_mat, n_energy=n_energy, voxel_nm=voxel, ewald=mode,
+               angles=(start, step, end), energies=np.sort(rng.uniform(250.0, 600.0, n_energy)))
+    # random aligned / isotropic pattern (tiny() makes only the last material isotropic)
+    mats = []
+    for m, (phi, S, th, ps) in enumerate(w.materials):
+        if S is not None and rng.random() < 0.35:
+            mats.append((phi, None, None, None))
+            w.delta_perp[:, m] = w.delta_par[:, m]; w.beta_perp[:, m] = w.beta_par[:, m]
+        else:
+            mats.append((phi, S, th, ps))
+    w.materials = mats
+    return w
+
+
+@pytest.mark.parametrize("i", range(48))
+def test_random_cases_match_oracle(i):
+    w = _random_case(i)
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, _ = _gpu(w, 0)
+    if ref.max() == 0.0:                                     # nothing on the Ewald sphere at all: exact zeros on both sides
+        assert (out == 0).all() and (cnt == rcnt).all()
+        return
+    compare(out, cnt, ref, rcnt, f"random {i}: {w.Nx}x{w.Ny}x{w.Nz}, {w.n_mat} materials, {w.n_energy} energies, {w.voxel_nm} nm")
