@@ -573,7 +573,7 @@ def test_A14_any_Nx_Ny_definition_dft_along_x_and_y():
     of Eq. 6 along such an axis.  Pins, none of which calls the routine it checks: the brute-force 3-D DFT,
     numpy's FFT (a library routine of the same definition), Parseval, a plane wave landing in exactly one bin with the
     forward sign, and the whole pipeline: a uniform isotropic film of odd size puts everything into q = 0 with the
-    closed-form value, and linear mode equals definition mode on 12 x 10 x 3."""
+    closed-form value, and linear mode equals definition mode on even, odd and mixed sizes (12 x 10 x 3, 9 x 7 x 3, ...)."""
     rng = np.random.default_rng(6)
     for shape in [(4, 6, 10), (3, 5, 7), (1, 12, 9), (2, 8, 6), (5, 4, 3)]:          # (Nz, Ny, Nx)
         f = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
@@ -601,10 +601,12 @@ def test_A14_any_Nx_Ny_definition_dft_along_x_and_y():
     assert np.isclose(img[0, ny // 2, nx // 2], expect, rtol=1e-10)
     rest = img[0].copy(); rest[ny // 2, nx // 2] = 0
     assert rest.max() < 1e-18 * expect
-    w = W.tiny(seed=78, nx=12, ny=10, nz=3, n_mat=2, n_energy=1, voxel_nm=1.5, ewald=W.EWALD_TRILINEAR)
-    a, ca = _run(w)
-    b, cb = _run(w, linear=True)
-    assert np.array_equal(ca, cb) and np.allclose(a, b, rtol=1e-11, atol=1e-14 * a.max())
+    # even, odd and mixed sizes (for odd N the bins run over -(N-1)/2 .. (N-1)/2 and q = 0 sits at pixel N/2, integer division)
+    for nx, ny, nz in [(12, 10, 3), (9, 7, 3), (8, 5, 1), (7, 12, 5)]:
+        w = W.tiny(seed=78 + nx, nx=nx, ny=ny, nz=nz, n_mat=2, n_energy=1, voxel_nm=1.5, ewald=W.EWALD_TRILINEAR)
+        a, ca = _run(w)
+        b, cb = _run(w, linear=True)
+        assert np.array_equal(ca, cb) and np.allclose(a, b, rtol=1e-11, atol=1e-14 * a.max()), (nx, ny, nz)
 
 
 # ================================================================ round-2 pins
