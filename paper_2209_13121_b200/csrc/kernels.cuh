@@ -344,6 +344,11 @@ struct EwaldBasisParams {
     const int *kind;            // [2 n_pack] BasisKind
 };
 
+#ifndef CYRSOXS_EW_PU
+#define CYRSOXS_EW_PU 4
+#endif
+constexpr int EW_PU = CYRSOXS_EW_PU;        // packs gathered per chunk in k_ewald_basis
+
 template <int EG>
 __global__ void __launch_bounds__(256)
 k_ewald_basis(const EwaldBasisParams q)
@@ -380,20 +385,35 @@ k_ewald_basis(const EwaldBasisParams q)
                 float2 c[NCHI];
 #pragma unroll
                 for (int f = 0; f < NCHI; ++f) c[f] = make_float2(0.f, 0.f);
-                for (int pk = 0; ok && pk < q.n_pack; ++pk, pq += fstride, pm += fstride) {
-                    const float2 z1 = __ldg(pq), z2 = __ldg(pm);
-                    // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
-                    const float2 F[2] = {make_float2(z1.x + z2.x, z1.y - z2.y), make_float2(z1.y + z2.y, z2.x - z1.x)};
+                // EW_PU packs at a time: the gathers of a chunk are issued before the first is used (the kernel is bound by the
+                // latency of these L2 gathers, ncu: long scoreboard 9 cycles per issue); same summation order.  Measured
+                // (CFG3 / CFG5 Ewald stage): one pack at a time 0.365 / 0.49 ms, four 0.314 / 0.406 ms; both nodes at once on
+                // top of that (120 registers, 2 CTAs per SM) 0.367 / 0.529 ms.
+                for (int pk0 = 0; ok && pk0 < q.n_pack; pk0 += EW_PU, pq += EW_PU * fstride, pm += EW_PU * fstride) {
+                    float2 z1[EW_PU], z2[EW_PU];
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const int kd = __ldg(q.kind + 2 * pk + h);
-                        const float2 v = cmul(__ldg(coef + 2 * pk + h), F[h]);
-                        if (kd == BK_PHI || kd == BK_W) { c[0] = cadd(c[0], v); c[3] = cadd(c[3], v); }
-                        else if (kd == BK_XX) c[0] = cadd(c[0], v);
-                        else if (kd == BK_YY) c[3] = cadd(c[3], v);
-                        else if (kd == BK_XY) c[1] = cadd(c[1], v);
-                        else if (kd == BK_XZ) c[2] = cadd(c[2], v);
-                        else if (kd == BK_YZ) c[4] = cadd(c[4], v);
+                    for (int u = 0; u < EW_PU; ++u) {
+                        const bool have = pk0 + u < q.n_pack;
+                        z1[u] = have ? __ldg(pq + u * fstride) : make_float2(0.f, 0.f);
+                        z2[u] = have ? __ldg(pm + u * fstride) : make_float2(0.f, 0.f);
+                    }
+#pragma unroll
+                    for (int u = 0; u < EW_PU; ++u) {
+                        const int pk = pk0 + u;
+                        // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
+                        const float2 F[2] = {make_float2(z1[u].x + z2[u].x, z1[u].y - z2[u].y), make_float2(z1[u].y + z2[u].y, z2[u].x - z1[u].x)};
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            if (pk >= q.n_pack) continue;                      // (uniform: the padding of the last chunk)
+                            const int kd = __ldg(q.kind + 2 * pk + h);
+                            const float2 v = cmul(__ldg(coef + 2 * pk + h), F[h]);
+                            if (kd == BK_PHI || kd == BK_W) { c[0] = cadd(c[0], v); c[3] = cadd(c[3], v); }
+                            else if (kd == BK_XX) c[0] = cadd(c[0], v);
+                            else if (kd == BK_YY) c[3] = cadd(c[3], v);
+                            else if (kd == BK_XY) c[1] = cadd(c[1], v);
+                            else if (kd == BK_XZ) c[2] = cadd(c[2], v);
+                            else if (kd == BK_YZ) c[4] = cadd(c[4], v);
+                        }
                     }
                 }
                 const float2 u[3] = {c[0], c[1], c[2]}, v[3] = {c[1], c[3], c[4]};
