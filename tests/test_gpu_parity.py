@@ -643,3 +643,24 @@ def test_random_cases_match_oracle(i):
         assert (out == 0).all() and (cnt == rcnt).all()
         return
     compare(out, cnt, ref, rcnt, f"random {i}: {w.Nx}x{w.Ny}x{w.Nz}, {w.n_mat} materials, {w.n_energy} energies, {w.voxel_nm} nm")
+
+
+@pytest.mark.parametrize("case", ["32 aligned materials", "300 energies", "360 angles", "32 materials 2-D"])
+def test_extreme_parameters(case):
+    """The ends of the accepted parameter ranges: n_mat = 32 all aligned (224 basis fields, 112 packs), 300 energies
+    (two energy batches of 256 + 44, three image-group widths), 360 angles (0:1:359), and 32 materials on a 2-D film (more
+    packs than the 2-D Ewald kernel's register file holds: the generic kernel takes over)."""
+    if case == "32 aligned materials":
+        w = W.tiny(seed=201, nx=64, ny=16, nz=4, n_mat=32, n_energy=2, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR, isotropic_last=False)
+    elif case == "300 energies":
+        w = W.tiny(seed=202, nx=32, ny=32, nz=2, n_mat=2, n_energy=300, voxel_nm=2.0, ewald=W.EWALD_NEAREST,
+                   energies=np.linspace(260.0, 700.0, 300))
+    elif case == "360 angles":
+        w = W.tiny(seed=203, nx=32, ny=16, nz=4, n_mat=2, n_energy=2, voxel_nm=1.0, ewald=W.EWALD_TRILINEAR, angles=(0.0, 1.0, 359.0))
+    else:
+        w = W.tiny(seed=204, nx=64, ny=64, nz=1, n_mat=32, n_energy=6, voxel_nm=2.0, ewald=W.EWALD_NEAREST)
+    ref, rcnt = oracle_run(w, linear=True)
+    out, cnt, ctx = _gpu(w, 0)
+    compare(out, cnt, ref, rcnt, case)
+    if case == "300 energies":
+        assert ctx.stats()["energy_batch"] == 256
