@@ -823,13 +823,14 @@ cyrsoxs_status run_batch_spectral(cyrsoxs_ctx *c, cudaStream_t st, int e0, int e
         p.wx = wx; p.wy = wy; p.wz = wz; p.pitch = pitch;
         p.spec = (const float2 *)c->A3.p; p.img = (float4 *)c->img.p;
         q.n_pack = c->n_pack; q.coef = (const float2 *)c->d_bcoef.p; q.kind = (const int *)c->d_bkind.p;
-        const size_t smem2d = (size_t)eb * (2 * sizeof(double) + sizeof(float) + 2 * c->n_pack * sizeof(float2)) + 2 * c->n_pack * sizeof(int);
-        if (c->Nz == 1 && eb >= 4 && c->n_pack <= EW2D_MAXP && smem2d <= 48 * 1024) {
+        const size_t smem2d = (size_t)eb * (2 * sizeof(double) + sizeof(float) + 2 * c->n_pack * sizeof(float2)) + 2 * c->n_pack * sizeof(int)
+                              + (size_t)2 * c->n_pack * 256 * sizeof(float2);
+        if (c->Nz == 1 && eb >= 4 && 2 * c->n_pack <= EW2D_MAXF && smem2d <= 96 * 1024) {
             // 2-D model, several energies: one thread per pixel, the batch's energies in an inner loop (see
             // k_ewald_basis_2d; cfg4 15.8 -> 6.6 ms; a single energy is better off with a thread per energy)
             const dim3 g2d((c->Nx + 31) / 32, (c->Ny + 7) / 8);
             switch (c->eg) {
-#define CASE(EG) case EG: launch_pdl(c->pdl, k_ewald_basis_2d<EG>, g2d, 256, smem2d, st, q); break;
+#define CASE(EG) case EG: if (cyrsoxs_status a = allow_smem(c, k_ewald_basis_2d<EG>, 96 * 1024)) return a; launch_pdl(c->pdl, k_ewald_basis_2d<EG>, g2d, 256, smem2d, st, q); break;
                 CASE(8) CASE(4) CASE(2) default: CASE(1)
 #undef CASE
             }

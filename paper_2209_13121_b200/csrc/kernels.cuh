@@ -427,13 +427,16 @@ k_ewald_basis(const EwaldBasisParams q)
     p.img[(((size_t)blockIdx.z * p.Ny + iy) * p.Nx + ix) * EG + sub] = make_float4(axx, ayy, axy, valid ? 1.f : 0.f);
 }
 
-// Ewald projection for SPECTRAL_BASIS on a 2-D model (Nz = 1, A13) with at most EW2D_MAXP packs: the
-// k_z = 0 plane serves every energy, so a thread owns one pixel, gathers and unpacks its basis
-// spectra once (registers) and loops over the batch's energies; per energy only the validity and
-// r-hat (fp64, same operation order as pixel_geometry), the coefficient sum and the projection
-// remain.  Coefficients, k, 1/k and k^4 of the batch sit in shared memory.  Same arithmetic and
-// summation order as k_ewald_basis: identical images.
-constexpr int EW2D_MAXP = 8;
+// Ewald projection for SPECTRAL_BASIS on a 2-D model (Nz = 1, A13): the k_z = 0 plane serves every energy, so a thread
+// owns one pixel, gathers and unpacks its basis spectra once and loops over the batch's energies; per energy only the
+// validity and r-hat (fp64, same operation order as pixel_geometry), the coefficient sum and the projection remain.
+// The unpacked fields F_b of the pixel sit in shared memory ([field][thread], conflict-free 64-bit accesses), which lets
+// the coefficient sum walk the basis MATERIAL BY MATERIAL (an aligned material is the run PHI, W, XX, YY, XY, XZ, YZ, an
+// isotropic one a single PHI; the kind table is only read to tell the two apart) with no per-field dispatch: round 1's
+// version kept F in registers, which forces compile-time field indices and a kind test per field and energy -- 388
+// thread-instructions per pixel and energy, 75 % of the issue slots (ncu r2_cfg4).  Coefficients, k, 1/k and k^4 of the
+// batch sit in shared memory too.  Same additions in the same order as k_ewald_basis: identical images.
+constexpr int EW2D_MAXF = 64;          // most basis fields (2 n_pack) the shared-memory layout is sized for
 
 template <int EG>
 __global__ void __launch_bounds__(256)
@@ -446,7 +449,8 @@ k_ewald_basis_2d(const EwaldBasisParams q)
     double *s_k = reinterpret_cast<double *>(smem_raw);              // [ne] k, then [ne] 1/k
     double *s_ik = s_k + ne;
     float2 *s_coef = reinterpret_cast<float2 *>(s_ik + ne);          // [ne][nb]
-    float *s_k4 = reinterpret_cast<float *>(s_coef + (size_t)ne * nb);   // [ne]
+    float2 *s_F = s_coef + (size_t)ne * nb;                           // [nb][256]
+    float *s_k4 = reinterpret_cast<float *>(s_F + (size_t)nb * 256);  // [ne]
     int *s_kind = reinterpret_cast<int *>(s_k4 + ne);                 // [nb]
     for (int e = threadIdx.x; e < ne; e += 256) {
         const double k = p.k[p.e0 + e];
@@ -456,26 +460,37 @@ k_ewald_basis_2d(const EwaldBasisParams q)
     }
     for (int i = threadIdx.x; i < ne * nb; i += 256) s_coef[i] = q.coef[(size_t)p.e0 * nb + i];
     for (int i = threadIdx.x; i < nb; i += 256) s_kind[i] = q.kind[i];
-    __syncthreads();
-    const int ix = blockIdx.x * 32 + (threadIdx.x & 31);
-    const int iy = blockIdx.y * 8 + (threadIdx.x >> 5);
-    if (ix >= p.Nx || iy >= p.Ny) return;
+    const int tid = threadIdx.x;
+    const int ix = blockIdx.x * 32 + (tid & 31);
+    const int iy = blockIdx.y * 8 + (tid >> 5);
+    const bool inside = ix < p.Nx && iy < p.Ny;
     const int mx = ix - p.Nx / 2, my = iy - p.Ny / 2;
     const int sx = win_slot(p.wx, mx), sy = win_slot(p.wy, my);
     const int tx = win_slot(p.wx, -mx), ty = win_slot(p.wy, -my);
-    const bool inwin = sx < p.wx.W && sy < p.wy.W && tx < p.wx.W && ty < p.wy.W;
+    const bool inwin = inside && sx < p.wx.W && sy < p.wy.W && tx < p.wx.W && ty < p.wy.W;
     const size_t fstride = (size_t)p.wy.W * p.pitch;                 // wz.W == 1
     const float2 *pq = p.spec + (size_t)sy * p.pitch + sx;
     const float2 *pm = p.spec + (size_t)ty * p.pitch + tx;
-    float2 F[2 * EW2D_MAXP];
+    float2 *F = s_F + tid;                                            // field b of this pixel at F[b * 256]
+    for (int pk0 = 0; pk0 < q.n_pack; pk0 += EW_PU) {                 // EW_PU packs' gathers in flight
+        float2 z1[EW_PU], z2[EW_PU];
 #pragma unroll
-    for (int pk = 0; pk < EW2D_MAXP; ++pk) {
-        float2 z1 = make_float2(0.f, 0.f), z2 = z1;
-        if (inwin && pk < q.n_pack) { z1 = __ldg(pq + pk * fstride); z2 = __ldg(pm + pk * fstride); }
-        // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
-        F[2 * pk] = make_float2(z1.x + z2.x, z1.y - z2.y);
-        F[2 * pk + 1] = make_float2(z1.y + z2.y, z2.x - z1.x);
+        for (int u = 0; u < EW_PU; ++u) {
+            const bool have = inwin && pk0 + u < q.n_pack;
+            z1[u] = have ? __ldg(pq + (size_t)(pk0 + u) * fstride) : make_float2(0.f, 0.f);
+            z2[u] = have ? __ldg(pm + (size_t)(pk0 + u) * fstride) : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < EW_PU; ++u) {
+            if (pk0 + u < q.n_pack) {
+                // Fa = z1 + conj z2, Fb = -i (z1 - conj z2)   (the 1/2 lives in coef)
+                F[(2 * (pk0 + u)) * 256] = make_float2(z1[u].x + z2[u].x, z1[u].y - z2[u].y);
+                F[(2 * (pk0 + u) + 1) * 256] = make_float2(z1[u].y + z2[u].y, z2[u].x - z1[u].x);
+            }
+        }
     }
+    __syncthreads();                                                  // the tables (F itself is private to the thread)
+    if (!inside) return;
     const double qx = __dmul_rn((double)mx, p.dqx), qy = __dmul_rn((double)my, p.dqy);
     const double qx2 = __dmul_rn(qx, qx), qy2 = __dmul_rn(qy, qy);
     const size_t pix = (size_t)iy * p.Nx + ix, plane = (size_t)p.Ny * p.Nx;
@@ -486,26 +501,27 @@ k_ewald_basis_2d(const EwaldBasisParams q)
         if (s2 >= 0.0) {
             const double ik = s_ik[e];
             const float r[3] = {(float)__dmul_rn(qx, ik), (float)__dmul_rn(qy, ik), (float)__dmul_rn(__dsqrt_rn(s2), ik)};
-            float2 c[NCHI];
-#pragma unroll
-            for (int f = 0; f < NCHI; ++f) c[f] = make_float2(0.f, 0.f);
+            float2 c0 = make_float2(0.f, 0.f), c1 = c0, c2 = c0, c3 = c0, c4 = c0;
             const float2 *coef = s_coef + (size_t)e * nb;
             if (inwin) {
-#pragma unroll
-                for (int b = 0; b < 2 * EW2D_MAXP; ++b) {
-                    if (b < nb) {
-                        const int kd = s_kind[b];
-                        const float2 v = cmul(coef[b], F[b]);
-                        if (kd == BK_PHI || kd == BK_W) { c[0] = cadd(c[0], v); c[3] = cadd(c[3], v); }
-                        else if (kd == BK_XX) c[0] = cadd(c[0], v);
-                        else if (kd == BK_YY) c[3] = cadd(c[3], v);
-                        else if (kd == BK_XY) c[1] = cadd(c[1], v);
-                        else if (kd == BK_XZ) c[2] = cadd(c[2], v);
-                        else if (kd == BK_YZ) c[4] = cadd(c[4], v);
-                    }
+                for (int b = 0; b < nb;) {
+                    const int kd = s_kind[b];
+                    if (kd == BK_NONE) { ++b; continue; }                         // padding of a pack / of a material group
+                    const bool aligned = b + 1 < nb && s_kind[b + 1] == BK_W;      // kd == BK_PHI starts a material
+                    float2 v = cmul(coef[b], F[b * 256]);                         // PHI
+                    c0 = cadd(c0, v); c3 = cadd(c3, v);
+                    if (aligned) {
+                        v = cmul(coef[b + 1], F[(b + 1) * 256]); c0 = cadd(c0, v); c3 = cadd(c3, v);      // W
+                        c0 = cadd(c0, cmul(coef[b + 2], F[(b + 2) * 256]));                                // XX
+                        c3 = cadd(c3, cmul(coef[b + 3], F[(b + 3) * 256]));                                // YY
+                        c1 = cadd(c1, cmul(coef[b + 4], F[(b + 4) * 256]));                                // XY
+                        c2 = cadd(c2, cmul(coef[b + 5], F[(b + 5) * 256]));                                // XZ
+                        c4 = cadd(c4, cmul(coef[b + 6], F[(b + 6) * 256]));                                // YZ
+                        b += 7;
+                    } else ++b;
                 }
             }
-            const float2 u[3] = {c[0], c[1], c[2]}, v3[3] = {c[1], c[3], c[4]};
+            const float2 u[3] = {c0, c1, c2}, v3[3] = {c1, c3, c4};
             float sxx, syy, sxy;
             project_pair(r, u, v3, sxx, syy, sxy);
             const float w = 1.f * s_k4[e];
