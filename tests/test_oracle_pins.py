@@ -421,6 +421,48 @@ def test_P10_binary_isotropic_film_closed_form_and_isi():
     assert max(r) / min(r) - 1 < 2e-2
 
 
+def test_P10_non_square_film_pins_dq_y_and_the_validity_ellipse():
+    """P10 on a 48 x 32 x 1 detector whose Ewald disk is cut by the detector edge (Eq. 7-8).
+    q_y = m_y 2 pi / (Ny voxel): with Nx != Ny the disk q_x^2 + q_y^2 <= k^2 is an ELLIPSE in pixels (k/dq_x = 17.65 px,
+    k/dq_y = 11.77 px) and r^_y enters the (1 - (r^.e)^2) factor with dq_y, so a dq_y formed from Nx changes both the
+    valid set and the values.  Everything on the right-hand side is written out in NumPy."""
+    rng = np.random.default_rng(48)
+    nx, ny, voxel, E = 48, 32, 1.6, 285.0
+    phi = (rng.integers(0, 257, (1, ny, nx)) / 256.0).astype(np.float32)
+    d1, b1, d2, b2 = 2.2e-3, 0.9e-3, 0.7e-3, 0.3e-3
+    f32 = lambda v: float(np.float32(v))
+    n1 = 1 - f32(d1) + 1j * f32(b1); n2 = 1 - f32(d2) + 1j * f32(b2)
+    k = 2 * PI * E / 1239.84197
+    dqx = 2 * PI / (nx * voxel); dqy = 2 * PI / (ny * voxel)
+    qx = (np.arange(nx) - nx // 2)[None, :] * dqx; qy = (np.arange(ny) - ny // 2)[:, None] * dqy
+    inside = qx ** 2 + qy ** 2 <= k ** 2
+    assert abs(k / dqx - 17.65) < 0.01 and abs(k / dqy - 11.77) < 0.01
+    assert 0 < inside.sum() < inside.size and not inside[0, nx // 2] and not inside[ny // 2, 0]     # cut on both axes
+    assert np.abs(qx ** 2 + qy ** 2 - k ** 2).min() > 1e-6 * k ** 2                                 # no pixel on the rim
+    wrong = qx ** 2 + ((np.arange(ny) - ny // 2)[:, None] * dqx) ** 2 <= k ** 2                     # the mistake this pins
+    assert (wrong != inside).sum() > 50
+    F = np.fft.fftshift(np.fft.fft2(phi[0].astype(np.float64)))
+    for z in (0.0, 40.0):
+        w = _iso_film(phi, d1, b1, d2, b2, voxel, E, (z, 0, z))
+        a, b, c = _consts(w)
+        assert abs(oracle.wavenumber(E) - k) <= 1e-15 * k
+        C, S = np.cos(np.deg2rad(z)), np.sin(np.deg2rad(z))
+        P = np.stack([oracle.fft3(x) for x in oracle.polarization(w.materials, a, b, c, (C, S, 0))])
+        for mode in (W.EWALD_NEAREST, W.EWALD_TRILINEAR):           # Nz = 1: both read the one k_z plane
+            img, valid = oracle.ewald(P, voxel, k, mode)
+            assert np.array_equal(valid.astype(bool), inside), (z, mode)
+            ref = k ** 4 * abs(n1 ** 2 - n2 ** 2) ** 2 / (16 * PI ** 2) * np.abs(F) ** 2 * (1 - ((qx * C + qy * S) / k) ** 2)
+            ref[ny // 2, nx // 2] = img[ny // 2, nx // 2]
+            assert np.abs(img - ref)[inside].max() <= 1e-12 * ref[inside].max(), (z, mode)
+            assert not img[~inside].any()
+    # the whole path on the same film (one angle, so the rotate step only resamples): total valid-pixel count is the ellipse's
+    w = _iso_film(phi, d1, b1, d2, b2, voxel, E, (0.0, 0, 0.0))
+    out, cnt = _run(w)
+    assert np.array_equal(cnt[0] > 0, inside)
+    assert np.abs(out[0] - np.where(inside, k ** 4 * abs(n1 ** 2 - n2 ** 2) ** 2 / (16 * PI ** 2) * np.abs(F) ** 2
+                                    * (1 - (qx / k) ** 2), 0.0))[inside & ~((qx == 0) & (qy == 0))].max() <= 1e-12 * out[0].max()
+
+
 # ---------------------------------------------------------------- P11 90-degree exactness
 
 def test_P11_rot90_of_sample_and_field():
