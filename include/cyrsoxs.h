@@ -237,6 +237,42 @@ cyrsoxs_status cyrsoxs_reduce(cyrsoxs_ctx *ctx, void *cuda_stream, const float *
                               const unsigned int *d_counts, int n_energy, int n_bins,
                               double sector_half_width_deg, float *d_I, float *d_A, float *d_isi);
 
+/* cyrsoxs_reduce for callers that must not allocate device memory.  Same arguments, same kernels and same results as
+ * cyrsoxs_reduce, but the per-bin sums the kernels need between their two
+ * launches live in a fixed array compiled into the library instead of a cudaMalloc'ed, context-owned buffer.
+ *
+ * Who needs it.  cudaMalloc can fail or hurt in a process that is otherwise healthy: (1) a host application (a PyTorch
+ * caching allocator, a reconstruction or fitting service at the beamline) that has already claimed the whole of HBM for
+ * its own pool, so any further cudaMalloc returns out-of-memory although the pool could have lent the bytes; (2) a
+ * live-analysis loop that reduces every detector frame as it arrives and cannot accept the device-wide synchronisation
+ * cudaMalloc and cudaFree imply, which stalls every other stream of the process for the length of the call.  Such
+ * callers create the context once at start-up, while allocating is still possible (cyrsoxs_create uploads a few KB of
+ * twiddle tables), and from then on use this call only: it performs no cudaMalloc, no cudaFree and calls no library
+ * routine that allocates; images and outputs are the caller's.
+ *
+ * Limits (INVALID_ARG with an explanatory cyrsoxs_last_error beyond them; use cyrsoxs_reduce for larger reductions):
+ *   1 <= n_bins <= CYRSOXS_REDUCE_STATIC_MAX_BINS, 1 <= n_energy <= CYRSOXS_REDUCE_STATIC_MAX_ENERGIES,
+ *   n_energy * n_bins <= CYRSOXS_REDUCE_STATIC_MAX_CELLS.
+ * The array is CYRSOXS_REDUCE_STATIC_BYTES (about 1.2 MB) of device memory on EVERY GPU on which the process uses this
+ * library, from the moment the library's code is loaded there until the process exits, whether or not this call is made.
+ *
+ * First call per device.  The first call on each GPU looks up the device address of the array (cudaGetSymbolAddress with
+ * that GPU current) and caches it; make that first call during start-up, outside any stream capture.  Later calls only
+ * enqueue one memset and two kernels on `cuda_stream`.
+ *
+ * Sharing.  There is ONE array per GPU, shared by every context and every call in the process, and it keeps what the last
+ * call left in it.  Each call therefore zeroes the part it uses, on `cuda_stream`, before its kernels run.  Two calls whose
+ * GPU work can overlap (different streams without an event between them, or two host threads) race on the array and
+ * produce garbage in both outputs: order them on one stream or with events.  Calls do not overlap with cyrsoxs_reduce's
+ * scratch, which is a different buffer. */
+#define CYRSOXS_REDUCE_STATIC_MAX_BINS 1024
+#define CYRSOXS_REDUCE_STATIC_MAX_ENERGIES 1024
+#define CYRSOXS_REDUCE_STATIC_MAX_CELLS 32768
+#define CYRSOXS_REDUCE_STATIC_BYTES (3 * 12 * CYRSOXS_REDUCE_STATIC_MAX_CELLS + 8 * CYRSOXS_REDUCE_STATIC_MAX_ENERGIES)
+cyrsoxs_status cyrsoxs_reduce_static(cyrsoxs_ctx *ctx, void *cuda_stream, const float *d_images,
+                                     const unsigned int *d_counts, int n_energy, int n_bins,
+                                     double sector_half_width_deg, float *d_I, float *d_A, float *d_isi);
+
 /* Test hook, not part of the contract: copies the per-energy Ewald images of the LAST energy
  * batch of the last run, as float4 (I_xx, I_yy, I_xy, valid) per pixel, for batch-local energy
  * index `e_in_batch`, into d_dst (Ny*Nx*4 floats, device).  Enqueued on the run's stream. */

@@ -15,6 +15,7 @@ LIB_PATH = PKG / "libcyrsoxs.so"
 OK, ERR_INVALID_ARG, ERR_NOT_READY, ERR_CUDA, ERR_OOM, ERR_NOT_IMPLEMENTED = range(6)
 EWALD_NEAREST, EWALD_TRILINEAR = 0, 1
 ALG_AUTO, ALG_PER_ENERGY, ALG_SPECTRAL_BASIS = 0, 1, 2
+REDUCE_STATIC_MAX_BINS, REDUCE_STATIC_MAX_ENERGIES, REDUCE_STATIC_MAX_CELLS = 1024, 1024, 32768   # include/cyrsoxs.h
 STAGES = ("xpass", "zpass", "ypass", "ewald", "rotate")
 N_STAGES = len(STAGES)
 
@@ -24,7 +25,7 @@ EXPORTS = [
     "cyrsoxs_set_counts_output", "cyrsoxs_set_profiling", "cyrsoxs_run", "cyrsoxs_num_angles",
     "cyrsoxs_set_spectra_shard", "cyrsoxs_set_energy_range", "cyrsoxs_run_spectra", "cyrsoxs_get_spectra", "cyrsoxs_get_spectra_part",
     "cyrsoxs_run_energies",
-    "cyrsoxs_get_stats", "cyrsoxs_reduce", "cyrsoxs_debug_fetch_images", "cyrsoxs_last_error", "cyrsoxs_destroy",
+    "cyrsoxs_get_stats", "cyrsoxs_reduce", "cyrsoxs_reduce_static", "cyrsoxs_debug_fetch_images", "cyrsoxs_last_error", "cyrsoxs_destroy",
     "cyrsoxs_version",
 ]
 
@@ -79,6 +80,7 @@ def load() -> C.CDLL:
     lib.cyrsoxs_get_stats.argtypes = [vp, C.POINTER(Stats)]
     lib.cyrsoxs_debug_fetch_images.argtypes = [vp, C.c_int, vp]
     lib.cyrsoxs_reduce.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, C.c_double, vp, vp, vp]
+    lib.cyrsoxs_reduce_static.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, C.c_double, vp, vp, vp]
     lib.cyrsoxs_last_error.argtypes = [vp]
     lib.cyrsoxs_last_error.restype = C.c_char_p
     lib.cyrsoxs_destroy.argtypes = [vp]
@@ -249,6 +251,15 @@ class Context:
                I_ptr: int, A_ptr: Optional[int] = None, isi_ptr: Optional[int] = None, stream: int = 0):
         self._check(self.lib.cyrsoxs_reduce(self.h, stream or None, images_ptr, counts_ptr or None, n_energy, n_bins,
                                             float(sector_half_width_deg), I_ptr, A_ptr or None, isi_ptr or None))
+
+    def reduce_static(self, images_ptr: int, counts_ptr: Optional[int], n_energy: int, n_bins: int, sector_half_width_deg: float,
+                      I_ptr: int, A_ptr: Optional[int] = None, isi_ptr: Optional[int] = None, stream: int = 0):
+        """cyrsoxs_reduce_static: `reduce` for callers that must not allocate device memory (another pool owns the HBM, or
+        cudaMalloc's device-wide synchronisation is unacceptable).  Scratch is a fixed array inside the library, shared by
+        all calls on a GPU: at most REDUCE_STATIC_MAX_BINS bins, REDUCE_STATIC_MAX_ENERGIES energies and
+        REDUCE_STATIC_MAX_CELLS energies x bins; calls that overlap on the GPU race (include/cyrsoxs.h)."""
+        self._check(self.lib.cyrsoxs_reduce_static(self.h, stream or None, images_ptr, counts_ptr or None, n_energy, n_bins,
+                                                   float(sector_half_width_deg), I_ptr, A_ptr or None, isi_ptr or None))
 
     def debug_fetch_images(self, e_in_batch: int, dst_ptr: int):
         self._check(self.lib.cyrsoxs_debug_fetch_images(self.h, e_in_batch, C.c_void_p(dst_ptr)))

@@ -10,6 +10,7 @@
 #include <string.h>
 #include <algorithm>
 #include <complex>
+#include <mutex>
 #include <string>
 #include <utility>
 #include <vector>
@@ -1460,6 +1461,98 @@ cyrsoxs_status cyrsoxs_reduce(cyrsoxs_ctx *c, void *cuda_stream, const float *d_
     const size_t smem = (size_t)3 * n_bins * (sizeof(double) + sizeof(unsigned int));
     if (smem > 48 * 1024)
         if (cyrsoxs_status a = allow_smem(c, k_reduce_accumulate, (size_t)3 * 4096 * 12)) return a;
+    k_reduce_accumulate<<<grid, 256, smem, st>>>(p);
+    CUDA_TRY(c, cudaGetLastError());
+    const int tot = n_energy * n_bins;
+    k_reduce_finalize<<<(tot + 255) / 256, 256, 0, st>>>(n_energy, n_bins, p.acc, p.num, p.total, c->dqx * c->dqy, d_I, d_A, d_isi);
+    CUDA_TRY(c, cudaGetLastError());
+    return CYRSOXS_OK;
+}
+
+} // extern "C"
+
+// ---- cyrsoxs_reduce_static: the reduction's scratch without cudaMalloc ------------------------------------------------
+// The per-bin sums, pixel counts and per-energy totals that k_reduce_accumulate hands to k_reduce_finalize normally sit
+// in c->red (cudaMalloc'ed on first use).  Callers that cannot allocate (HBM already owned by another pool, or no
+// tolerance for cudaMalloc's device-wide synchronisation; see include/cyrsoxs.h) get the same two kernels pointed at this
+// array instead.  It is part of the library's device image: every GPU that loads the library holds
+// CYRSOXS_REDUCE_STATIC_BYTES for it until the process exits.
+//
+// In HOST code the name g_reduce_static is only a handle for the runtime's symbol calls, NOT a device address: giving
+// `g_reduce_static` (or &g_reduce_static[0]) to a kernel faults, or on systems where the GPU can reach host memory quietly
+// works on the wrong bytes.  The address each device uses comes from cudaGetSymbolAddress, asked once per device with that
+// device current (reduce_static_address below) and then passed to the kernels like any other pointer.
+static __device__ __align__(256) unsigned char g_reduce_static[CYRSOXS_REDUCE_STATIC_BYTES];
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+std::mutex g_reduce_static_mutex;                    // contexts of different host threads may reach the table together
+void *g_reduce_static_ptr[kMaxDevices] = {};          // device address of g_reduce_static on device i, nullptr = not asked yet
+
+// Device address of g_reduce_static on the context's device, which the caller has made current.  The first call per
+// device asks the runtime (this may load the library's device code there: keep it out of stream captures); later calls
+// read the table.
+cyrsoxs_status reduce_static_address(cyrsoxs_ctx *c, void **out)
+{
+    if (c->device < 0 || c->device >= kMaxDevices) return fail(c, CYRSOXS_ERR_INVALID_ARG, "reduce_static: device index %d beyond %d", c->device, kMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_reduce_static_mutex);
+    if (!g_reduce_static_ptr[c->device]) {
+        int cur = -1;
+        CUDA_TRY(c, cudaGetDevice(&cur));
+        if (cur != c->device) return fail(c, CYRSOXS_ERR_CUDA, "reduce_static: device %d could not be made current (current: %d)", c->device, cur);
+        void *ptr = nullptr;
+        CUDA_TRY(c, cudaGetSymbolAddress(&ptr, g_reduce_static));
+        if (!ptr) return fail(c, CYRSOXS_ERR_CUDA, "reduce_static: cudaGetSymbolAddress returned a null address");
+        g_reduce_static_ptr[c->device] = ptr;
+    }
+    *out = g_reduce_static_ptr[c->device];
+    return CYRSOXS_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+cyrsoxs_status cyrsoxs_reduce_static(cyrsoxs_ctx *c, void *cuda_stream, const float *d_images, const unsigned int *d_counts,
+                                     int n_energy, int n_bins, double sector_half_width_deg, float *d_I, float *d_A, float *d_isi)
+{
+    if (!c) return CYRSOXS_ERR_INVALID_ARG;
+    if (!d_images || !d_I) return fail(c, CYRSOXS_ERR_INVALID_ARG, "reduce_static: images or I output is NULL");
+    if (n_energy < 1 || n_bins < 1) return fail(c, CYRSOXS_ERR_INVALID_ARG, "reduce_static: n_energy >= 1 and n_bins >= 1");
+    if (n_bins > CYRSOXS_REDUCE_STATIC_MAX_BINS || n_energy > CYRSOXS_REDUCE_STATIC_MAX_ENERGIES
+        || (long long)n_energy * n_bins > CYRSOXS_REDUCE_STATIC_MAX_CELLS)
+        return fail(c, CYRSOXS_ERR_INVALID_ARG,
+                    "reduce_static: %d energies x %d bins exceed the fixed scratch (at most %d bins, %d energies, %d energies x bins); "
+                    "use cyrsoxs_reduce, which allocates", n_energy, n_bins, CYRSOXS_REDUCE_STATIC_MAX_BINS,
+                    CYRSOXS_REDUCE_STATIC_MAX_ENERGIES, CYRSOXS_REDUCE_STATIC_MAX_CELLS);
+    if (!(sector_half_width_deg > 0.0) || !(sector_half_width_deg <= 45.0))
+        return fail(c, CYRSOXS_ERR_INVALID_ARG, "reduce_static: sector half width must be in (0, 45] degrees");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DeviceGuard guard(c->device);
+    void *scratch = nullptr;
+    if (cyrsoxs_status s = reduce_static_address(c, &scratch)) return s;
+    // same layout as cyrsoxs_reduce inside its buffer: [e][3][bins] double sums, [e] double totals, [e][3][bins] counts
+    const size_t nb = (size_t)n_energy * 3 * n_bins;
+    const size_t bytes = sizeof(double) * nb + sizeof(double) * n_energy + sizeof(unsigned int) * nb;
+    static_assert(sizeof(double) * 3 * CYRSOXS_REDUCE_STATIC_MAX_CELLS + sizeof(double) * CYRSOXS_REDUCE_STATIC_MAX_ENERGIES
+                      + sizeof(unsigned int) * 3 * CYRSOXS_REDUCE_STATIC_MAX_CELLS == CYRSOXS_REDUCE_STATIC_BYTES,
+                  "the limits of include/cyrsoxs.h size the array");
+    // the array still holds the previous call's sums (any context, any stream): the kernels add into it, so zero what
+    // this call uses, stream-ordered before them
+    CUDA_TRY(c, cudaMemsetAsync(scratch, 0, bytes, st));
+    ReduceParams p{};
+    p.Nx = c->Nx; p.Ny = c->Ny; p.n_bins = n_bins;
+    p.rho = (double)c->Nx / (double)c->Ny;
+    p.tan_w = tan(sector_half_width_deg * (kPi / 180.0));
+    p.img = d_images; p.cnt = d_counts;
+    p.acc = (double *)scratch; p.total = p.acc + nb; p.num = (unsigned int *)(p.total + n_energy);
+    const int want = std::max(1, 4 * c->n_sm / n_energy);
+    p.rows_per_cta = std::max(4, (c->Ny + want - 1) / want);
+    const dim3 grid((c->Ny + p.rows_per_cta - 1) / p.rows_per_cta, n_energy);
+    // 36 KB at the bin limit: below the 48 KB a kernel may use without raising its attribute
+    const size_t smem = (size_t)3 * n_bins * (sizeof(double) + sizeof(unsigned int));
+    static_assert((size_t)3 * CYRSOXS_REDUCE_STATIC_MAX_BINS * 12 <= 48 * 1024, "bin limit keeps the default shared-memory size");
     k_reduce_accumulate<<<grid, 256, smem, st>>>(p);
     CUDA_TRY(c, cudaGetLastError());
     const int tot = n_energy * n_bins;
