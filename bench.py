@@ -265,15 +265,17 @@ def measure(name, args, rank, world, dev, steps, warmup, with_e2e, with_clocks, 
         n_parts = min(world, w.n_mat)
         a_e, b_e = sharding.energy_slices(w.n_energy, world)[rank]
         ctx.set_spectra_shard(rank % n_parts, n_parts)
-        ctx.set_energy_range(a_e, max(b_e - a_e, 1))
-        out = torch.empty((max(b_e - a_e, 1), w.Ny, w.Nx), dtype=torch.float32, device=dev)
+        if b_e > a_e:
+            ctx.set_energy_range(a_e, b_e - a_e)
+        # more ranks than energies: this rank transforms and exchanges but has no energy of its own (zero-row `out`)
+        out = torch.empty((b_e - a_e, w.Ny, w.Nx), dtype=torch.float32, device=dev)
 
     def one_step():
         flush.fill_(1)                                  # L2 flush between timed iterations (outside the events)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
         if strong:
-            sharding.run_strong(ctx, w, out, sptr)
+            sharding.run_strong(ctx, w, out, sptr, device=dev.index)
         else:
             ctx.run(out.data_ptr(), sptr)
         b.record(stream)
@@ -370,6 +372,28 @@ def roofline_of(name, res, peak, peak_src):
     # SURVEY.md 8(d) contract model M0: (16 c + 96) bytes per voxel per energy (+28 per pixel in 2-D)
     m0_bytes = w.n_energy * ((16.0 * w.n_mat + 96.0) * w.n_vox + (28.0 * w.Nx * w.Ny if w.Nz == 1 else 0.0))
     traffic, traffic_src = ncu_traffic(name, dom)
+    if dom_stages == ["rotate"]:
+        # The rotate/average kernel is not an HBM kernel (DRAM 3 % busy at CFG4): its binding resource is the L1 data pipe,
+        # one 128-byte wavefront per clock and SM (DESIGN 7.4).  Algorithmic work per launch: pixels x energies x angles
+        # bilinear samples, 4 taps each, a warp-wide tap of 16-byte texels = 32 x 16 / 128 = 4 wavefronts.
+        import torch
+        n_sm = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+        sm_mhz = float((res.get("clocks") or {}).get("sm_max_mhz") or 1965.0)
+        wavefronts = float(w.Nx) * w.Ny * w.n_energy * w.n_angles * 4.0 / 32.0 * 4.0 / dom_launches
+        l1_peak = n_sm * sm_mhz * 1e6 / 1e9                          # G wavefronts/s
+        l1_ach = wavefronts / (dom_ms_per_launch * 1e-3) / 1e9 if dom_ms_per_launch > 0 else 0.0
+        return {"bound": "l1", "kernel": dom, "stages": dom_stages, "launches_per_step": dom_launches,
+                "share_of_step": ktime[dom] / max(sum(ktime.values()), 1e-12),
+                "achieved": l1_ach, "peak": l1_peak, "unit": "Gwavefront/s", "frac": l1_ach / l1_peak,
+                "peak_source": f"L1 data pipe: 1 wavefront (128 B) per clock and SM x {n_sm} SMs x {sm_mhz:.0f} MHz (DESIGN 7.4)",
+                "wavefronts_per_launch": wavefronts, "floor_ms_per_launch": wavefronts / (l1_peak * 1e9) * 1e3,
+                "traffic": traffic, "traffic_source": traffic_src, "limiter": groups[dom][1],
+                "hbm_frac": achieved / peak, "bytes_per_launch": dom_bytes_per_launch, "ms_per_launch": dom_ms_per_launch,
+                "stage_ms_per_step": stage_ms,
+                "stage_gbs": {k: (st["stage_bytes"][k] / (stage_ms[k] * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0) for k in stage_ms},
+                "whole_step": {"bytes": whole_bytes, "achieved": whole_bytes / (ms * 1e-3) / 1e9, "frac": whole_bytes / (ms * 1e-3) / 1e9 / peak},
+                "whole_step_vs_M0": {"bytes": m0_bytes, "achieved": m0_bytes / (ms * 1e-3) / 1e9, "frac": m0_bytes / (ms * 1e-3) / 1e9 / peak,
+                                     "note": "M0 = (16c+96) B/voxel/energy (SURVEY 8(d))"}}
     return {"bound": "hbm", "kernel": dom, "stages": dom_stages, "launches_per_step": dom_launches,
             "share_of_step": ktime[dom] / max(sum(ktime.values()), 1e-12),
             "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_vs_nominal_8000": achieved / 8000.0,
@@ -506,7 +530,8 @@ def run_ours(args, rank, world, local_rank):
             wo = r["w"]
             per[other] = {"workload": workload_label(wo, other), "ms_per_step": r["ms_per_step"],
                           "patterns_per_s": wo.n_energy * wo.n_angles / (r["ms_per_step"] * 1e-3),
-                          "dominant_kernel": rf["kernel"], "frac": rf["frac"], "traffic": rf["traffic"],
+                          "dominant_kernel": rf["kernel"], "bound": rf["bound"], "frac": rf["frac"], "unit": rf["unit"],
+                          "ms_per_launch": rf["ms_per_launch"], "traffic": rf["traffic"],
                           "stage_ms_per_step": rf["stage_ms_per_step"], "cufft_comparison": cufft_comparison(wo, dev, r["stage_ms"]),
                           "whole_step_frac": rf["whole_step"]["frac"], "whole_step_vs_M0_frac": rf["whole_step_vs_M0"]["frac"]}
             del r, wo

@@ -107,7 +107,13 @@ cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, double voxel_nm
  * isotropic material (S == 0); d_S, d_theta, d_psi themselves may be NULL if every material
  * is isotropic.  Pointers are BORROWED: the caller keeps the arrays alive and unmodified until
  * every run that uses them has completed.  Arrays must be 16-byte aligned.  The library does
- * not check sum_m phi_m = 1 (neither does the paper's code) nor clamp S. */
+ * not check sum_m phi_m = 1 (neither does the paper's code) nor clamp S.
+ * Angle range: SPECTRAL_BASIS forms sin and cos of theta and psi with the hardware approximation
+ * (about 5e-7 absolute) and no extended range reduction, which holds for |angle| up to a few pi
+ * (tests cover [-3 pi, 3 pi]); beyond that the error of each director component grows by about
+ * 6e-8 |angle| (3e-6 at 50 rad: images then agree with a double-precision evaluation to about
+ * 1e-4 instead of 1e-5).  Wrap angles into [-pi, pi] on the caller's side if they can be large.
+ * PER_ENERGY uses sincosf, accurate at any magnitude. */
 cyrsoxs_status cyrsoxs_set_morphology(cyrsoxs_ctx *ctx, const float *const *d_phi,
                                       const float *const *d_S, const float *const *d_theta,
                                       const float *const *d_psi);
@@ -193,7 +199,9 @@ int cyrsoxs_num_angles(const cyrsoxs_ctx *ctx);
  *       field count (7 fields per aligned material, 1 per isotropic one; 1 <= n_parts <= n_mat); this context transforms
  *       group `part` only.  The fields of a group are paired among themselves (an odd count is padded), so the pack layout
  *       depends on n_parts, not on `part`: every GPU that sets the same n_parts has the same layout.  Needs a resident
- *       morphology and SPECTRAL_BASIS (else NOT_IMPLEMENTED at run).  (0, 1) restores the unsharded layout.
+ *       morphology and SPECTRAL_BASIS (else NOT_IMPLEMENTED at run).  (0, 1) restores the unsharded layout.  A shard
+ *       divides the transform WORK, not the workspace: every context still holds the x- and z-pass buffers and the
+ *       spectra buffer for all packs (the other parts' spectra are copied into the latter).
  *   cyrsoxs_set_energy_range(ctx, first, count)     phase 2 (and cyrsoxs_run) processes energies [first, first + count)
  *       of the tables given to cyrsoxs_set_optical_constants; `out` and the counts buffer then hold `count` images.  The
  *       spectral windows are always sized for ALL energies of the tables, so GPUs with different ranges share one layout.
@@ -205,7 +213,8 @@ int cyrsoxs_num_angles(const cyrsoxs_ctx *ctx);
  *       a part owns.  The caller copies the other parts' blocks in (NCCL broadcast / all_gather, or cudaMemcpyPeer),
  *       ordered after phase 1 and before phase 2 on the streams it uses.
  *   cyrsoxs_run_energies(ctx, stream, out)          phase 2 on whatever the spectra buffer holds (NOT_READY unless
- *       cyrsoxs_run_spectra ran after the last change of morphology, constants or shard).
+ *       cyrsoxs_run_spectra ran, under SPECTRAL_BASIS, after the last change of morphology, constants, shard or
+ *       algorithm, and no PER_ENERGY run has overwritten the buffer since).
  * cyrsoxs_run is phase 1 followed by phase 2; with a shard of more than one part it produces images from this part's
  * materials only, so sharded callers use the two calls.  PER_ENERGY: phase 1 is empty, phase 2 does everything. */
 cyrsoxs_status cyrsoxs_set_spectra_shard(cyrsoxs_ctx *ctx, int part, int n_parts);

@@ -92,7 +92,7 @@ struct cyrsoxs_ctx {
     unsigned long long null_pattern = ~0ull;
     // workspace
     DevBuf A1, A2, A3, img, twx, twy, twz, stage_out[2], red;
-    DevBuf tw2x, tw2y, tw2z;                     // per-stage twiddle tables of fft2.cuh (lengths 64 .. 2048)
+    DevBuf tw2x;                                 // per-stage twiddle tables of fft2.cuh for the x pass (lengths 64 .. 2048)
     // last run
     cyrsoxs_stats stats{};
     cudaStream_t last_stream = nullptr;
@@ -551,7 +551,7 @@ cyrsoxs_status run_batch_per_energy(cyrsoxs_ctx *c, cudaStream_t st, int e0, int
         }
         CUDA_TRY(c, cudaGetLastError());
         const double nodes = (c->Nz > 1 && c->ewald == CYRSOXS_EWALD_TRILINEAR) ? 2.0 : 1.0;
-        c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * 0.785 * nodes * NCHI * 8.0 + 16.0 * c->Nx * c->Ny);
+        c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * (kPi / 4.0) * nodes * NCHI * 8.0 + 16.0 * c->Nx * c->Ny);
     }
     return launch_rotate(c, st, e0, eb, d_out, d_cnt);
 }
@@ -826,7 +826,8 @@ cyrsoxs_status run_batch_spectral(cyrsoxs_ctx *c, cudaStream_t st, int e0, int e
         q.n_pack = c->n_pack; q.coef = (const float2 *)c->d_bcoef.p; q.kind = (const int *)c->d_bkind.p;
         const size_t smem2d = (size_t)eb * (2 * sizeof(double) + sizeof(float) + 2 * c->n_pack * sizeof(float2)) + 2 * c->n_pack * sizeof(int)
                               + (size_t)2 * c->n_pack * 256 * sizeof(float2);
-        if (c->Nz == 1 && eb >= 4 && 2 * c->n_pack <= EW2D_MAXF && smem2d <= 96 * 1024) {
+        const bool two_d = c->Nz == 1 && eb >= 4 && 2 * c->n_pack <= EW2D_MAXF && smem2d <= 96 * 1024;
+        if (two_d) {
             // 2-D model, several energies: one thread per pixel, the batch's energies in an inner loop (see
             // k_ewald_basis_2d; cfg4 15.8 -> 6.6 ms; a single energy is better off with a thread per energy)
             const dim3 g2d((c->Nx + 31) / 32, (c->Ny + 7) / 8);
@@ -844,7 +845,11 @@ cyrsoxs_status run_batch_spectral(cyrsoxs_ctx *c, cudaStream_t st, int e0, int e
         }
         CUDA_TRY(c, cudaGetLastError());
         const double nodes = (c->Nz > 1 && c->ewald == CYRSOXS_EWALD_TRILINEAR) ? 2.0 : 1.0;
-        c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += eb * ((double)wx.W * wy.W * 0.785 * nodes * 2.0 * c->n_pack * 8.0 + 16.0 * c->Nx * c->Ny);
+        // gather: the valid disk's share (pi/4) of the spectral window, both partner bins of every pack; the 2-D kernel
+        // gathers once per BATCH (its energies loop over the unpacked fields in shared memory), the 3-D one per energy.
+        // Plus one float4 image per pixel and energy.
+        const double gather = (double)wx.W * wy.W * (kPi / 4.0) * nodes * 2.0 * c->n_pack * 8.0;
+        c->stats.stage_bytes[CYRSOXS_STAGE_EWALD] += (two_d ? 1.0 : (double)eb) * gather + (double)eb * 16.0 * c->Nx * c->Ny;
     }
     return launch_rotate(c, st, e0, eb, d_out, d_cnt);
 }
@@ -879,8 +884,7 @@ cyrsoxs_status cyrsoxs_create(int Nx, int Ny, int Nz, int n_mat, double voxel_nm
     if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); c->n_sm = 148; }
     cyrsoxs_status st;
     if ((st = make_twiddles(c, c->twx, Nx)) != CYRSOXS_OK || (st = make_twiddles(c, c->twy, Ny)) != CYRSOXS_OK
-        || (st = make_twiddles(c, c->twz, Nz)) != CYRSOXS_OK || (st = make_twiddles2(c, c->tw2x, Nx)) != CYRSOXS_OK
-        || (st = make_twiddles2(c, c->tw2y, Ny)) != CYRSOXS_OK || (st = make_twiddles2(c, c->tw2z, Nz)) != CYRSOXS_OK) {
+        || (st = make_twiddles(c, c->twz, Nz)) != CYRSOXS_OK || (st = make_twiddles2(c, c->tw2x, Nx)) != CYRSOXS_OK) {
         cyrsoxs_destroy(c);
         return st;
     }
@@ -895,7 +899,7 @@ void cyrsoxs_destroy(cyrsoxs_ctx *c)
     cudaDeviceSynchronize();                 // nothing of this context may still be running when its buffers go
     clear_prof(c);
     for (void *p : c->owned_morph) cudaFree(p);
-    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->d_tiles[4], &c->d_tiles[5], &c->d_tiles[6], &c->d_tiles[7], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz, &c->tw2x, &c->tw2y, &c->tw2z,
+    for (DevBuf *b : {&c->d_coef, &c->d_k, &c->d_reach2, &c->d_cs, &c->d_csf, &c->d_tiles[0], &c->d_tiles[1], &c->d_tiles[2], &c->d_tiles[3], &c->d_tiles[4], &c->d_tiles[5], &c->d_tiles[6], &c->d_tiles[7], &c->A1, &c->A2, &c->A3, &c->img, &c->twx, &c->twy, &c->twz, &c->tw2x,
                       &c->stage_out[0], &c->stage_out[1], &c->d_bcoef, &c->d_bkind, &c->d_bmat, &c->red})
         release(*b);
     release(c->stage_morph[0]); release(c->stage_morph[1]);
@@ -1198,6 +1202,7 @@ cyrsoxs_status cyrsoxs_set_algorithm(cyrsoxs_ctx *c, cyrsoxs_algorithm alg)
     if (!c) return CYRSOXS_ERR_INVALID_ARG;
     if (alg != CYRSOXS_ALG_AUTO && alg != CYRSOXS_ALG_PER_ENERGY && alg != CYRSOXS_ALG_SPECTRAL_BASIS)
         return fail(c, CYRSOXS_ERR_INVALID_ARG, "unknown algorithm");
+    if (alg != c->alg) c->spectra_ready = false;     // spectra of a run under another setting are not handed to run_energies
     c->alg = alg;
     return CYRSOXS_OK;
 }
@@ -1221,7 +1226,22 @@ int cyrsoxs_num_angles(const cyrsoxs_ctx *c) { return c && c->have_angles ? c->n
 // phases: 1 = the energy-independent spectra (SPECTRAL_BASIS), 2 = the energies of the range; cyrsoxs_run does both
 enum { PHASE_SPECTRA = 1, PHASE_ENERGIES = 2 };
 
+static cyrsoxs_status run_body(cyrsoxs_ctx *c, void *cuda_stream, float *out, int phases);
+
+// A run that fails partway may already have enqueued work on `cuda_stream` that uses the shared workspace: mark the end of
+// that partial work too, so that the next run on ANOTHER stream still waits for it (ev_run_done pairs with last_stream).
 static cyrsoxs_status run_impl(cyrsoxs_ctx *c, void *cuda_stream, float *out, int phases)
+{
+    const cyrsoxs_status s = run_body(c, cuda_stream, out, phases);
+    if (s != CYRSOXS_OK && c && c->ev_run_done && c->last_stream == (cudaStream_t)cuda_stream) {
+        DeviceGuard guard(c->device);
+        if (cudaEventRecord(c->ev_run_done, c->last_stream) == cudaSuccess) c->ran = true;
+        else cudaGetLastError();
+    }
+    return s;
+}
+
+static cyrsoxs_status run_body(cyrsoxs_ctx *c, void *cuda_stream, float *out, int phases)
 {
     if (!c) return CYRSOXS_ERR_INVALID_ARG;
     if ((phases & PHASE_ENERGIES) && !out) return fail(c, CYRSOXS_ERR_INVALID_ARG, "out is NULL");
@@ -1233,6 +1253,7 @@ static cyrsoxs_status run_impl(cyrsoxs_ctx *c, void *cuda_stream, float *out, in
     if (!c->ev_run_done) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_run_done, cudaEventDisableTiming));
     // the workspace and the device tables are shared by consecutive runs: a run on another stream waits for the last one
     if (c->ran && st != c->last_stream) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_run_done, 0));
+    c->last_stream = st;             // from here on everything this call enqueues is on st (run_impl marks its end, also on failure)
 
     // where does `out` live?
     bool out_on_host = false;
@@ -1284,7 +1305,7 @@ static cyrsoxs_status run_impl(cyrsoxs_ctx *c, void *cuda_stream, float *out, in
     const size_t fixed = (spectral ? sizeof(float2) * (a1 + a2 + a3) : 0) + stage_bytes;
     // The energy batch depends on the free device memory; cudaMemGetInfo is slow, so the batch is
     // re-planned only when what it depends on has changed since the last run.
-    if (c->shard_parts > 1 && !spectral)
+    if (c->shard_parts > 1 && (!spectral || c->streamed))
         return fail(c, CYRSOXS_ERR_NOT_IMPLEMENTED, "a spectra shard needs CYRSOXS_ALG_SPECTRAL_BASIS (or AUTO) and a resident morphology");
     const unsigned long long plan_key = (unsigned long long)nE_run * 8 + (spectral ? 4 : 0) + (out_on_host ? 2 : 0) + 1;
     int eb = c->plan_eb;
@@ -1334,11 +1355,16 @@ static cyrsoxs_status run_impl(cyrsoxs_ctx *c, void *cuda_stream, float *out, in
     c->stats.workspace_bytes = (double)(c->A1.cap + c->A2.cap + c->A3.cap + c->img.cap + c->stage_out[0].cap + c->stage_out[1].cap);
     c->last_stream = st;
 
-    if (phases & PHASE_SPECTRA) {
-        if (spectral && (s = run_basis_spectra(c, st, wx, wy, wz, pitch)) != CYRSOXS_OK) return s;
+    // spectra_ready means "A3 holds the basis spectra of the current configuration": only the spectral path sets it, and a
+    // PER_ENERGY run, whose phase 1 is empty and whose phase 2 fills A1..A3 with per-energy chi spectra, takes it away
+    if (!spectral)
+        c->spectra_ready = false;
+    else if (phases & PHASE_SPECTRA) {
+        c->spectra_ready = false;
+        if ((s = run_basis_spectra(c, st, wx, wy, wz, pitch)) != CYRSOXS_OK) return s;
         c->spectra_ready = true;
-    } else if (spectral && !c->spectra_ready)
-        return fail(c, CYRSOXS_ERR_NOT_READY, "cyrsoxs_run_energies needs cyrsoxs_run_spectra first (after the last change of morphology, constants or shard)");
+    } else if (!c->spectra_ready)
+        return fail(c, CYRSOXS_ERR_NOT_READY, "cyrsoxs_run_energies needs cyrsoxs_run_spectra first (after the last change of morphology, constants, shard or algorithm)");
 
     int nb = 0;
     for (int e0 = e_first; (phases & PHASE_ENERGIES) && e0 < e_first + nE_run; e0 += eb, ++nb) {

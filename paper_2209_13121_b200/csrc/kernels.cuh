@@ -30,7 +30,7 @@ __device__ __forceinline__ void pdl_entry()
 struct Window {
     int N, lo, W;
 };
-// (N a power of two for x and y; the z axis may have any length, DESIGN 3-A14)
+// (every axis may have any length up to 2048, DESIGN 3-A14; powers of two take the FFT kernels)
 __host__ __device__ __forceinline__ int win_slot(const Window &w, int k)
 {
     const int d = k - w.lo;
@@ -604,7 +604,7 @@ k_rotate_avg(const RotateParams p)
     const float4 *img = p.img + (size_t)g0 * plane + sub;
     const double rho = p.rho;
     const double u = (double)(ix - p.Nx / 2), v = (double)(iy - p.Ny / 2);
-    const double vr = v * rho, ur = u / rho;                 // exact: rho is a power of two
+    const double vr = v * rho, ur = u / rho;                 // each rounded once, as in the oracle (rho = Nx/Ny need not be a power of two)
     const double cx = (double)(p.Nx / 2), cy = (double)(p.Ny / 2);
     const double xmax = (double)(p.Nx - 1), ymax = (double)(p.Ny - 1);
     const float r2 = (float)(u * u + vr * vr);

@@ -1,5 +1,6 @@
-// kernels2.cuh -- second-generation FFT passes built on fft_reg.cuh (register-first /
-// register-last): the strided z / y pass (k_col2) and the SPECTRAL_BASIS x pass (k_xbasis2).
+// kernels2.cuh -- second-generation FFT passes built on fft_reg.cuh / fft2.cuh (register-first /
+// register-last): the strided z / y passes (k_col2, k_col2p), the SPECTRAL_BASIS x passes (k_xbasis3; k_xbasis2
+// below 64 points) and the direct-DFT passes for lengths that are not powers of two (k_coldft, k_xdft).
 #pragma once
 #include "fft_reg.cuh"
 #include "fft2.cuh"
@@ -140,8 +141,8 @@ k_col2p(const ColParams p)
     }
 }
 
-// Strided pass for a length that is not a power of two (the z axis only: the paper uses Nz = 63,
-// P:459): the definition of Eq. 6 evaluated directly, and only at the window's bins -- the "direct DFT
+// Strided pass (z or y axis) for a length that is not a power of two (the paper uses Nz = 63, P:459;
+// lateral sizes of any length since DESIGN 3-A14): the definition of Eq. 6 evaluated directly, and only at the window's bins -- the "direct DFT
 // at the k_z bins the Ewald pixels need" north_star allows.  A CTA stages a tile of TX columns by N rows
 // and the twiddle table in shared memory; thread (c, og) accumulates bins s = og, og + OG, ... of column c.
 // The phase index k z mod N is stepped in exact integer arithmetic.  O(W N) per column: meant for the

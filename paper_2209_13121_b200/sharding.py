@@ -154,17 +154,28 @@ class _DevicePtr:
         self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
 
 
-def spectra_tensor(ctx):
-    """The context-owned spectra buffer as a [n_pack, pack_bytes] uint8 CUDA tensor (no copy)."""
+def spectra_tensor(ctx, device=None):
+    """The context-owned spectra buffer as a [n_pack, pack_bytes] uint8 CUDA tensor (no copy).  `device`: index of the
+    GPU the context was created on (default: torch's current device -- pass it when that may differ)."""
     import torch
     ptr, pack_bytes, n_pack = ctx.spectra()
-    return torch.as_tensor(_DevicePtr(ptr, pack_bytes * n_pack), device="cuda").view(n_pack, pack_bytes)
+    dev = torch.device("cuda", torch.cuda.current_device() if device is None else int(device))
+    return torch.as_tensor(_DevicePtr(ptr, pack_bytes * n_pack), device=dev).view(n_pack, pack_bytes)
 
 
-def run_strong(ctx, workload, out, stream_ptr: int, group=None):
+def run_strong(ctx, workload, out, stream_ptr: int, group=None, device=None):
     """One strong-scaling run on this rank: its part of the spectra, the exchange, its slice of the energies into
     `out` [n_local][Ny][Nx].  `ctx` has the full morphology, ALL energies of the workload, angles and Ewald mode set,
-    its shard set to (rank % n_parts, n_parts) and its energy range to the rank's slice.  Returns bytes received."""
+    its shard set to (rank % n_parts, n_parts) and, unless the rank's slice is empty, its energy range set to that slice.
+    A rank with an empty slice (more ranks than energies) passes `out` with zero rows (or None): it still transforms and
+    exchanges, and skips the energy phase.  `stream_ptr` is the cudaStream_t everything is ordered on: the broadcasts
+    of the exchange are issued with that stream current (NCCL orders a collective after the current stream's work), so
+    they sit between cyrsoxs_run_spectra and cyrsoxs_run_energies whatever stream the caller has current.  `device`:
+    index of the context's GPU (default: torch's current device).  Returns bytes received.  Not yet run on more than one
+    physical GPU."""
+    import contextlib
+
+    import torch
     import torch.distributed as dist
     world = dist.get_world_size(group) if dist.is_initialized() else 1
     ctx.run_spectra(stream_ptr)
@@ -172,10 +183,15 @@ def run_strong(ctx, workload, out, stream_ptr: int, group=None):
     if world > 1:
         aligned = [m[1] is not None for m in workload.materials]
         n_parts = min(world, len(aligned))
-        spec = spectra_tensor(ctx)
+        dev = torch.cuda.current_device() if device is None else int(device)
+        spec = spectra_tensor(ctx, dev)
         ranges = [ctx.spectra_part(q) for q in range(n_parts)]
         assert ranges == pack_ranges(aligned, n_parts), "library and host disagree on the pack layout"
-        received = exchange_spectra(spec, ranges, group)          # on torch's current stream == the run's stream
+        on_run_stream = contextlib.nullcontext()
+        if torch.cuda.current_stream(dev).cuda_stream != int(stream_ptr or 0):
+            on_run_stream = torch.cuda.stream(torch.cuda.ExternalStream(int(stream_ptr), device=dev))
+        with on_run_stream:
+            received = exchange_spectra(spec, ranges, group)
     if out is not None and out.shape[0] > 0:
         ctx.run_energies(out.data_ptr(), stream_ptr)
     return received

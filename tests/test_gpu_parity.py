@@ -174,11 +174,12 @@ def test_cfg5_quarter_depth_sampled_energies():
 
 @pytest.mark.skipif(_host_ram_gb() < 100.0 or os.environ.get("CYRSOXS_SKIP_FULL_CFG5") == "1",
                     reason="full CFG5 needs ~90 GB of host RAM for the generator and the oracle (about 80 s on the B200 box)")
-def test_cfg5_full_size_first_and_last_energy():
+def test_cfg5_full_size_five_energies():
     """BASELINE configs[4] at full size (1024x1024x512 = 5.4e8 voxels, 17 GB of morphology): 64-bit indexing, memory
-    footprint, the largest windows (last energy) and the low-k end (first energy)."""
+    footprint, the largest windows (last energy), the low-k end (first energy) and three energies in between -- five
+    Ewald geometries of the 20 on the configuration the bench line is quoted on (about 40 s of oracle time each)."""
     w = W.cfg5()
-    _full_size_sampled(w, [0, 19], "cfg5")
+    _full_size_sampled(w, [0, 5, 10, 15, 19], "cfg5")
 
 
 @pytest.mark.parametrize("alg", ALGS)
@@ -314,6 +315,9 @@ def test_aos_morphology_matches_soa():
     ctx.run(out.data_ptr(), s)
     torch.cuda.synchronize()
     assert torch.equal(out, ref[0])
+    # ... and against the oracle, fed from the SoA arrays the Real4 array was packed from (not only against the SoA GPU run)
+    oref, ocnt = oracle_run(w)
+    compare(out.cpu().numpy(), None, oref, ocnt, "aos-vs-oracle")
     # the isotropic last material was detected: same transform count as the SoA run
     assert ctx.stats()["stage_bytes"]["xpass"] == ref[-1].stats()["stage_bytes"]["xpass"]
     with pytest.raises(binding.CyrsoxsError):
@@ -382,8 +386,14 @@ def test_streamed_morphology_matches_oracle(group, nx):
     with pytest.raises(binding.CyrsoxsError) as ei:
         ctx.run(out.data_ptr(), s)
     assert ei.value.status == binding.ERR_NOT_IMPLEMENTED
-    # back to a resident morphology on the same context
+    # a spectra shard needs a resident morphology (cyrsoxs.h): refused, not silently ignored
     ctx.set_algorithm(binding.ALG_AUTO)
+    ctx.set_spectra_shard(1, 2)
+    with pytest.raises(binding.CyrsoxsError) as ei:
+        ctx.run_spectra(s)
+    assert ei.value.status == binding.ERR_NOT_IMPLEMENTED
+    ctx.set_spectra_shard(0, 1)
+    # back to a resident morphology on the same context
     ctx.set_morphology_host(w.materials, s)
     ctx.run(out.data_ptr(), s)
     torch.cuda.synchronize()
@@ -603,6 +613,76 @@ def test_spectra_shards_and_energy_ranges_match_oracle(n_mat, n_parts):
     compare(out[:3].cpu().numpy(), None, ref[1:4], rcnt[1:4], "energy range 1..3")
     for c in ctxs + [fresh]:
         c.close()
+
+
+def test_spectra_do_not_survive_an_algorithm_switch():
+    """cyrsoxs_run_energies only accepts spectra that the SPECTRAL_BASIS path produced under the current setting: under
+    PER_ENERGY phase 1 is empty and phase 2 leaves per-energy chi spectra in the same buffer, so switching the algorithm
+    between the phases must give NOT_READY (also for cyrsoxs_get_spectra), not images from the wrong buffer."""
+    import torch
+    from paper_2209_13121_b200 import binding
+    w = W.tiny(seed=77, nx=32, ny=32, nz=8, n_mat=2, n_energy=3, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR)
+    ref, rcnt = oracle_run(w)
+    s = torch.cuda.current_stream().cuda_stream
+    mats = [tuple(None if a is None else torch.from_numpy(a).cuda() for a in m) for m in w.materials]
+    ctx = binding.Context(w.Nx, w.Ny, w.Nz, w.n_mat, w.voxel_nm)
+    ctx.set_morphology(mats)
+    ctx.set_optical_constants(w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp)
+    ctx.set_angles(*w.angles); ctx.set_ewald(w.ewald)
+    out = torch.empty((w.n_energy, w.Ny, w.Nx), dtype=torch.float32, device="cuda")
+
+    def refused(fn):
+        with pytest.raises(binding.CyrsoxsError) as ei:
+            fn()
+        assert ei.value.status == binding.ERR_NOT_READY
+
+    # PER_ENERGY: run_spectra is a no-op, a whole run fills the buffers with chi spectra -- neither makes spectra "ready"
+    ctx.set_algorithm(binding.ALG_PER_ENERGY)
+    ctx.run_spectra(s)
+    refused(ctx.spectra)
+    ctx.run(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    compare(out.cpu().numpy(), None, ref, rcnt, "per-energy")
+    ctx.set_algorithm(binding.ALG_SPECTRAL_BASIS)
+    refused(lambda: ctx.run_energies(out.data_ptr(), s))
+    refused(ctx.spectra)
+    # the regular two-phase sequence works, and a later PER_ENERGY run takes the spectra away again
+    ctx.run_spectra(s)
+    out.zero_()
+    ctx.run_energies(out.data_ptr(), s)
+    torch.cuda.synchronize()
+    compare(out.cpu().numpy(), None, ref, rcnt, "two-phase")
+    ctx.set_algorithm(binding.ALG_PER_ENERGY)
+    ctx.set_algorithm(binding.ALG_SPECTRAL_BASIS)
+    refused(lambda: ctx.run_energies(out.data_ptr(), s))
+    ctx.close()
+
+
+def test_director_angles_of_tens_of_radians():
+    """cyrsoxs.h states the angle range: SPECTRAL_BASIS takes sin/cos of theta and psi from the hardware approximation
+    without extended range reduction, so unwrapped angles of tens of radians cost accuracy (about 6e-8 |angle| per
+    director component) but nothing worse; PER_ENERGY (sincosf) keeps the full gates.  The oracle gets the same float32
+    angles and evaluates them in double."""
+    w = W.tiny(seed=88, nx=32, ny=32, nz=8, n_mat=3, n_energy=2, voxel_nm=2.0, ewald=W.EWALD_TRILINEAR)
+    rng = np.random.default_rng(88)
+    mats = []
+    for phi, S, th, ps in w.materials:
+        if S is None:
+            mats.append((phi, S, th, ps))
+        else:       # same directors, unwrapped by random multiples of 2 pi up to +-8 turns (|angle| up to 56 rad)
+            turns = lambda: rng.integers(-8, 9, phi.shape).astype(np.float64) * 2.0 * np.pi
+            mats.append((phi, S, (th.astype(np.float64) + turns()).astype(np.float32), (ps.astype(np.float64) + turns()).astype(np.float32)))
+    w2 = W.Workload("unwrapped", w.Nx, w.Ny, w.Nz, w.voxel_nm, mats, w.energies, w.delta_par, w.beta_par, w.delta_perp, w.beta_perp,
+                    w.angles, w.ewald)
+    ref, rcnt = oracle_run(w2)
+    out, cnt, _ = _gpu(w2, 1)                                   # PER_ENERGY: full gates
+    compare(out, cnt, ref, rcnt, "unwrapped per-energy")
+    out, cnt, _ = _gpu(w2, 2)                                   # SPECTRAL_BASIS: the documented degradation, no more
+    assert np.isfinite(out).all() and np.array_equal(cnt, rcnt)
+    for e in range(w2.n_energy):
+        l2 = np.linalg.norm(out[e] - ref[e]) / np.linalg.norm(ref[e])
+        assert l2 <= 2e-4, (e, l2)
+        print("unwrapped spectral-basis e", e, "relative L2", l2)
 
 
 def _random_case(i):
